@@ -1,0 +1,173 @@
+/* fpm.h -- C-ABI boundary of the B200-native FastPM particle-mesh step.
+ *
+ * One GPU, one stream, no collectives.  Every entry point follows the paper's statement of the
+ * problem (FlowPM, arxiv 2010.11847; citations are PAPER.md:LINE) and SURVEY.md section 8(b).
+ *
+ * Conventions common to all calls
+ *   - Return value: FPM_OK (0) or a negative fpm_status.  Argument validation is synchronous and
+ *     has no side effects.  CUDA errors are sticky per context: once FPM_ECUDA is returned every
+ *     later call on that context returns FPM_ECUDA; fpm_last_error() gives the text.  No
+ *     exception crosses this boundary and the library never calls exit().
+ *   - Unless a parameter is marked HOST, every array argument is a DEVICE pointer owned by the
+ *     caller (e.g. a torch tensor's data_ptr()); the library never allocates, frees or keeps it.
+ *     Scratch memory is also caller-owned: query fpm_workspace_bytes(), allocate, hand it over
+ *     with fpm_set_workspace().  Only small plan tables (twiddles, per-axis kernel tables) are
+ *     owned by the context.
+ *   - All work is enqueued on the context's CUDA stream and the call returns without
+ *     synchronising (except the *_host calls, which synchronise before returning).
+ *   - Layouts.  Particles are structure-of-arrays: pos/mom/force are 3 contiguous planes
+ *     [3][n] of float32; positions are in MESH-CELL units, wrapped to [0, ng); momenta are
+ *     p = a^2 dx/dt / H0 in mesh cells.  Real meshes are [ng][ng][ng] float32, z fastest.
+ *     k-space meshes are [ng][ng][ng/2+1] interleaved complex64 (the cuFFT r2c layout), integer
+ *     frequency n_d in (-ng/2, ng/2], omega_d = 2 pi n_d / ng.
+ *   - Sizes: ng and np are powers of two, 8 <= np <= ng <= 1024, ng % np == 0.
+ */
+#ifndef FPM_H
+#define FPM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  FPM_OK = 0,
+  FPM_EINVAL = -1,   /* bad argument (null pointer, size, alignment, mode) */
+  FPM_ENOMEM = -2,   /* workspace missing or too small */
+  FPM_ECUDA = -3,    /* a CUDA call or kernel launch failed (sticky) */
+  FPM_ENOTIMPL = -4
+} fpm_status;
+
+/* Transfer function nabla nabla^-2 (Eq. 3-5). */
+enum {
+  FPM_KERNEL_PAPER = 0, /* Eq. 4 (3-point Laplacian symbol) + Eq. 5 (4-point gradient) [default] */
+  FPM_KERNEL_NAIVE = 1, /* -1/k^2 and i k ("the simplest way") */
+  FPM_KERNEL_MIXED = 2  /* -1/k^2 and Eq. 5 */
+};
+
+/* Kick/drift operators (Eq. 1-2). */
+enum {
+  FPM_FACTORS_FASTPM = 0, /* growth-factor form (exact for a Zel'dovich flow) [default] */
+  FPM_FACTORS_QUINN = 1   /* plain integrals  int da/(a^3 E), int da/(a^2 E) */
+};
+
+/* How the three force components are produced inside fpm_force / fpm_nbody. */
+enum {
+  FPM_FORCE_UNFUSED = 0, /* r2c, apply_force_kernel, 3x c2r, 3x readout as separate kernels */
+  FPM_FORCE_FUSED = 1    /* Green's function fused into the FFT passes, readout+kick+drift fused */
+};
+
+typedef struct {
+  int32_t ng;          /* mesh cells per side */
+  int32_t np;          /* particles per side (np^3 particles on a lattice of spacing ng/np) */
+  double omega_m;      /* flat LCDM: E(a)^2 = omega_m a^-3 + 1 - omega_m */
+  double box;          /* Mpc/h, bookkeeping only */
+  int32_t kernel_mode; /* FPM_KERNEL_* */
+  int32_t factor_mode; /* FPM_FACTORS_* */
+  int32_t force_path;  /* FPM_FORCE_* */
+  int32_t reserved;    /* must be 0 */
+} fpm_config;
+
+typedef struct fpm_ctx fpm_ctx;
+
+/* ---- context ---------------------------------------------------------------------------- */
+const char* fpm_version(void);
+
+/* cfg: HOST.  cuda_stream: a cudaStream_t (NULL = legacy default stream).  *out receives the
+ * context.  FPM_EINVAL on bad sizes/modes, FPM_ECUDA if the plan tables cannot be created. */
+int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out);
+int fpm_destroy(fpm_ctx* ctx);
+/* Text of the last error on this context (HOST string owned by the context; "" if none). */
+const char* fpm_last_error(const fpm_ctx* ctx);
+
+/* Bytes of scratch needed by fpm_force / fpm_nbody / fpm_lpt_init / the adjoint driver for this
+ * configuration (0 on invalid cfg).  The single-operator calls (paint, readout, fft, kick, drift,
+ * apply_force_kernel, *_adjoint) need no workspace. */
+size_t fpm_workspace_bytes(const fpm_config* cfg);
+/* ws: DEVICE, 256-byte aligned, stays owned by the caller and must outlive its use. */
+int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes);
+
+/* ---- background cosmology (host, float64; paper defers to Feng et al. 2016) -- */
+/* out: HOST double[7] = {D1, f1, D2, f2, E, Gf = a^3 E dD1/da, gf = dGf/da}, D1(1) = 1. */
+int fpm_growth(const fpm_ctx* ctx, double a, double* out);
+/* Drift factor multiplying p (epoch a_c) to move x from a_i to a_f; kick factor multiplying the
+ * force (epoch a_c) to move p from a_i to a_f.  HOST doubles. */
+int fpm_drift_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out);
+int fpm_kick_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out);
+
+/* ---- the operators of one PM step --------------------------------------------------------- */
+
+/* Cloud-in-cell paint: mesh[c] = sum_p m_p prod_d max(0, 1 - |x_pd - c_d|),
+ * periodic.  pos [3][n]; mass [n] or NULL (=> every particle has mass (ng/np)^3 so <mesh> = 1);
+ * mesh [ng^3] is OVERWRITTEN.  n >= 0. */
+int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, float* mesh);
+
+/* 3-D real-to-complex FFT: cplx(k) = sum_x real(x) exp(-2 pi i n.x/ng),
+ * unnormalised.  real [ng^3] is read only; cplx [ng*ng*(ng/2+1)] complex64 (float2). */
+int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx);
+/* Inverse: real(x) = ng^-3 sum_k cplx(k) exp(+2 pi i n.x/ng), with the
+ * Hermitian half implied.  cplx is CLOBBERED (used as scratch for the in-place passes). */
+int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real);
+
+/* Transfer function (Eq. 3-5): fk_d = scale * i g(omega_d) delta_k / K^2,
+ * 1/K^2 := 0 at k = 0, g := 0 at the Nyquist index of axis d.  Outputs must not alias delta_k. */
+int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, float* fkx,
+                           float* fky, float* fkz);
+
+/* Cloud-in-cell readout, same window as paint: out[p] = sum_c mesh[c] W(x_p - c). */
+int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, float* out);
+
+/* One force evaluation at the particles (Alg. 3 ForceGrids local, between a
+ * paint and three readouts): force [3][n] = -1.5 omega_m grad laplace^-1 delta at pos, i.e. already
+ * multiplied by 1.5 omega_m.  Needs the workspace.  The painted density stays in the workspace
+ * (fpm_workspace_density) until the next call. */
+int fpm_force(fpm_ctx* ctx, const float* pos, int64_t n, float* force);
+/* DEVICE pointer to the [ng^3] density painted by the last fpm_force / fpm_nbody force evaluation
+ * (valid only with FPM_FORCE_UNFUSED or right after fpm_paint_density); NULL without workspace. */
+const float* fpm_workspace_density(const fpm_ctx* ctx);
+
+/* Kick (Eq. 2): mom += force * K(ai, ac, af); force [3][n] already holds 1.5 omega_m. */
+int fpm_kick(fpm_ctx* ctx, float* mom, const float* force, int64_t n, double ai, double ac,
+             double af);
+/* Drift (Eq. 1): pos = wrap(pos + mom * D(ai, ac, af)) into [0, ng). */
+int fpm_drift(fpm_ctx* ctx, float* pos, const float* mom, int64_t n, double ai, double ac,
+              double af);
+
+/* ---- initial conditions and the whole run -------------------------------------------------- */
+
+/* LPT initial conditions (Alg. 4).  delta_lin [np^3]: real-space Gaussian
+ * linear field at a = 1 on the particle lattice.  order 1 (Zel'dovich) or 2.  Outputs pos, mom
+ * [3][np^3] in mesh cells at scale factor a0.  Needs the workspace. */
+int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, float* pos,
+                 float* mom);
+
+/* Whole FastPM run (PAPER.md:37-45 leapfrog).  a_stages: HOST double
+ * [n_steps+1] (a_0 .. a_n).  Force at a_0, then per step: half kick to sqrt(a_j a_j+1), drift to
+ * a_j+1, force, half kick.  pos/mom [3][n] are updated in place, n = np^3.  traj: NULL, or DEVICE
+ * [(n_steps+1)][3][n] receiving the positions at every force evaluation (for the backward pass).
+ * Needs the workspace. */
+int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int n_steps,
+              float* traj);
+
+/* The same run with HOST buffers: h_pos/h_mom [3][n] (pinned or pageable) are copied to the
+ * device buffers d_pos/d_mom (DEVICE, caller-owned), evolved, copied back; synchronises. */
+int fpm_nbody_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom,
+                   const double* a_stages, int n_steps);
+
+/* ---- adjoints ("differentiable with respect to every component") ------ */
+
+/* VJP of paint.  grad_mesh [ng^3] = dL/dmesh.  grad_pos [3][n] = m_p sum_c grad_mesh[c] dW/dx_d
+ * (overwritten); grad_mass [n] = readout(grad_mesh) (overwritten) or NULL. */
+int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n,
+                      const float* grad_mesh, float* grad_pos, float* grad_mass);
+/* VJP of readout.  grad_out [n] = dL/dout.  grad_mesh [ng^3] is ACCUMULATED INTO (+= paint of
+ * grad_out); grad_pos [3][n] = grad_out_p sum_c mesh[c] dW/dx_d (overwritten) or NULL. */
+int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n,
+                        const float* grad_out, float* grad_mesh, float* grad_pos);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FPM_H */

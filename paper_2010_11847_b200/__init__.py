@@ -1,0 +1,244 @@
+"""Thin Python binding of libfpm (include/fpm.h): argument marshalling only.
+
+Every numerical step runs in the CUDA kernels of libfpm.so; PyTorch supplies device memory and
+the stream.  There is no CPU fallback: importing this package without the built library, or
+calling it with CPU tensors, raises.
+"""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libfpm.so")
+
+KERNEL_PAPER, KERNEL_NAIVE, KERNEL_MIXED = 0, 1, 2
+FACTORS_FASTPM, FACTORS_QUINN = 0, 1
+FORCE_UNFUSED, FORCE_FUSED = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ENOTIMPL = 0, -1, -2, -3, -4
+
+
+class FpmError(RuntimeError):
+    pass
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [("ng", ctypes.c_int32), ("np", ctypes.c_int32), ("omega_m", ctypes.c_double),
+                ("box", ctypes.c_double), ("kernel_mode", ctypes.c_int32),
+                ("factor_mode", ctypes.c_int32), ("force_path", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+
+def _load():
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2010_11847_b200.build` "
+            "(nvcc, sm_100a). There is no CPU fallback.")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, i64, dbl, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+    sig = {
+        "fpm_version": (ctypes.c_char_p, []),
+        "fpm_create": (i32, [ctypes.POINTER(_Config), vp, ctypes.POINTER(vp)]),
+        "fpm_destroy": (i32, [vp]),
+        "fpm_last_error": (ctypes.c_char_p, [vp]),
+        "fpm_workspace_bytes": (ctypes.c_size_t, [ctypes.POINTER(_Config)]),
+        "fpm_set_workspace": (i32, [vp, vp, ctypes.c_size_t]),
+        "fpm_growth": (i32, [vp, dbl, ctypes.POINTER(dbl)]),
+        "fpm_drift_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
+        "fpm_kick_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
+        "fpm_paint": (i32, [vp, vp, vp, i64, vp]),
+        "fpm_fft_r2c": (i32, [vp, vp, vp]),
+        "fpm_fft_c2r": (i32, [vp, vp, vp]),
+        "fpm_apply_force_kernel": (i32, [vp, vp, ctypes.c_float, vp, vp, vp]),
+        "fpm_readout": (i32, [vp, vp, vp, i64, vp]),
+        "fpm_force": (i32, [vp, vp, i64, vp]),
+        "fpm_workspace_density": (vp, [vp]),
+        "fpm_kick": (i32, [vp, vp, vp, i64, dbl, dbl, dbl]),
+        "fpm_drift": (i32, [vp, vp, vp, i64, dbl, dbl, dbl]),
+        "fpm_lpt_init": (i32, [vp, vp, dbl, i32, vp, vp]),
+        "fpm_nbody": (i32, [vp, vp, vp, ctypes.POINTER(dbl), i32, vp]),
+        "fpm_nbody_host": (i32, [vp, vp, vp, vp, vp, ctypes.POINTER(dbl), i32]),
+        "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
+        "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+_lib = _load()
+
+
+def version():
+    return _lib.fpm_version().decode()
+
+
+def library_path():
+    return _LIB_PATH
+
+
+def _dev(t, dtype=torch.float32):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise FpmError(f"expected a contiguous CUDA {dtype} tensor (no CPU fallback), got "
+                       f"{type(t).__name__} {getattr(t, 'dtype', None)} {getattr(t, 'device', None)}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class FPM:
+    """One context = one (ng, np, cosmology, kernel) configuration on one CUDA stream."""
+
+    def __init__(self, ng, np_side=None, omega_m=0.3075, box=0.0, kernel_mode=KERNEL_PAPER,
+                 factor_mode=FACTORS_FASTPM, force_path=FORCE_UNFUSED, device="cuda:0",
+                 stream=None, workspace=True):
+        if not torch.cuda.is_available():
+            raise FpmError("CUDA device required: libfpm has no CPU fallback")
+        self.device = torch.device(device)
+        self.ng, self.np_side = int(ng), int(np_side if np_side is not None else ng)
+        self.n_particles = self.np_side ** 3
+        self.nzh = self.ng // 2 + 1
+        self.omega_m = float(omega_m)
+        self._cfg = _Config(self.ng, self.np_side, self.omega_m, float(box), kernel_mode,
+                            factor_mode, force_path, 0)
+        with torch.cuda.device(self.device):
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = ctypes.c_void_p()
+            rc = _lib.fpm_create(ctypes.byref(self._cfg), ctypes.c_void_p(self._stream.cuda_stream),
+                                 ctypes.byref(h))
+        if rc != OK:
+            raise FpmError(f"fpm_create failed with status {rc}")
+        self._h = h
+        self._ws = None
+        if workspace:
+            nbytes = _lib.fpm_workspace_bytes(ctypes.byref(self._cfg))
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            off = (-self._ws.data_ptr()) % 256
+            self._check(_lib.fpm_set_workspace(self._h, ctypes.c_void_p(self._ws.data_ptr() + off), nbytes))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.fpm_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != OK:
+            raise FpmError(f"libfpm status {rc}: {_lib.fpm_last_error(self._h).decode()}")
+
+    def _empty(self, *shape, dtype=torch.float32):
+        return torch.empty(*shape, dtype=dtype, device=self.device)
+
+    # ---- cosmology ----------------------------------------------------------------------
+    def growth(self, a):
+        out = (ctypes.c_double * 7)()
+        self._check(_lib.fpm_growth(self._h, a, out))
+        return dict(zip(("D1", "f1", "D2", "f2", "E", "Gf", "gf"), list(out)))
+
+    def drift_factor(self, ai, ac, af):
+        out = ctypes.c_double()
+        self._check(_lib.fpm_drift_factor(self._h, ai, ac, af, ctypes.byref(out)))
+        return out.value
+
+    def kick_factor(self, ai, ac, af):
+        out = ctypes.c_double()
+        self._check(_lib.fpm_kick_factor(self._h, ai, ac, af, ctypes.byref(out)))
+        return out.value
+
+    # ---- operators ------------------------------------------------------------------------
+    def paint(self, pos, mass=None, out=None):
+        n = pos.shape[1]
+        mesh = out if out is not None else self._empty(self.ng, self.ng, self.ng)
+        self._check(_lib.fpm_paint(self._h, _dev(pos), _dev(mass), n, _dev(mesh)))
+        return mesh
+
+    def fft_r2c(self, real, out=None):
+        cplx = out if out is not None else self._empty(self.ng, self.ng, self.nzh, dtype=torch.complex64)
+        self._check(_lib.fpm_fft_r2c(self._h, _dev(real), _dev(cplx, torch.complex64)))
+        return cplx
+
+    def fft_c2r(self, cplx, out=None, clobber=False):
+        work = cplx if clobber else cplx.clone()
+        real = out if out is not None else self._empty(self.ng, self.ng, self.ng)
+        self._check(_lib.fpm_fft_c2r(self._h, _dev(work, torch.complex64), _dev(real)))
+        return real
+
+    def apply_force_kernel(self, delta_k, scale=1.0):
+        outs = [torch.empty_like(delta_k) for _ in range(3)]
+        self._check(_lib.fpm_apply_force_kernel(self._h, _dev(delta_k, torch.complex64), scale,
+                                                *[_dev(o, torch.complex64) for o in outs]))
+        return outs
+
+    def readout(self, mesh, pos):
+        n = pos.shape[1]
+        out = self._empty(n)
+        self._check(_lib.fpm_readout(self._h, _dev(mesh), _dev(pos), n, _dev(out)))
+        return out
+
+    def force(self, pos):
+        n = pos.shape[1]
+        f = self._empty(3, n)
+        self._check(_lib.fpm_force(self._h, _dev(pos), n, _dev(f)))
+        return f
+
+    def workspace_density(self):
+        """Copy of the density painted by the last force evaluation (unfused path)."""
+        ptr = _lib.fpm_workspace_density(self._h)
+        if not ptr:
+            raise FpmError("no workspace")
+        out = self._empty(self.ng, self.ng, self.ng)
+        off = ptr - self._ws.data_ptr()
+        out.view(-1).copy_(self._ws[off:off + out.numel() * 4].view(torch.float32))
+        return out
+
+    def kick(self, mom, force, ai, ac, af):
+        self._check(_lib.fpm_kick(self._h, _dev(mom), _dev(force), mom.shape[1], ai, ac, af))
+        return mom
+
+    def drift(self, pos, mom, ai, ac, af):
+        self._check(_lib.fpm_drift(self._h, _dev(pos), _dev(mom), pos.shape[1], ai, ac, af))
+        return pos
+
+    def lpt_init(self, delta_lin, a0, order):
+        pos, mom = self._empty(3, self.n_particles), self._empty(3, self.n_particles)
+        self._check(_lib.fpm_lpt_init(self._h, _dev(delta_lin), a0, order, _dev(pos), _dev(mom)))
+        return pos, mom
+
+    def nbody(self, pos, mom, stages, traj=None):
+        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+        self._check(_lib.fpm_nbody(self._h, _dev(pos), _dev(mom), st, len(stages) - 1, _dev(traj)))
+        return pos, mom
+
+    def nbody_host(self, h_pos, h_mom, d_pos, d_mom, stages):
+        """Whole run on HOST float32 tensors (pinned for full PCIe speed); synchronises."""
+        for t in (h_pos, h_mom):
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+                raise FpmError("nbody_host expects contiguous CPU float32 tensors")
+        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+        self._check(_lib.fpm_nbody_host(self._h, ctypes.c_void_p(h_pos.data_ptr()),
+                                        ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos), _dev(d_mom),
+                                        st, len(stages) - 1))
+        return h_pos, h_mom
+
+    def paint_adjoint(self, pos, grad_mesh, mass=None, want_grad_mass=True):
+        n = pos.shape[1]
+        gpos = self._empty(3, n)
+        gmass = self._empty(n) if want_grad_mass else None
+        self._check(_lib.fpm_paint_adjoint(self._h, _dev(pos), _dev(mass), n, _dev(grad_mesh),
+                                           _dev(gpos), _dev(gmass)))
+        return gpos, gmass
+
+    def readout_adjoint(self, mesh, pos, grad_out, grad_mesh=None, want_grad_pos=True):
+        n = pos.shape[1]
+        gm = grad_mesh if grad_mesh is not None else torch.zeros(self.ng, self.ng, self.ng,
+                                                                  dtype=torch.float32, device=self.device)
+        gpos = self._empty(3, n) if want_grad_pos else None
+        self._check(_lib.fpm_readout_adjoint(self._h, _dev(mesh), _dev(pos), n, _dev(grad_out),
+                                             _dev(gm), _dev(gpos)))
+        return gm, gpos

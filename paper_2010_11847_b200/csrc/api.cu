@@ -1,0 +1,373 @@
+// api.cu -- the C-ABI of libfpm (include/fpm.h): validation, context, workspace carving and the
+// step / run / initial-condition drivers.  Every numerical step runs in the kernels of this
+// library (fft.cu, mesh_ops.cu, green.cu, particles.cu); there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "fpm_internal.h"
+
+using namespace fpm;
+
+namespace {
+
+inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
+inline size_t real_bytes(int n) { return align256(sizeof(float) * (size_t)n * n * n); }
+inline size_t cplx_bytes(int n) { return align256(sizeof(float2) * (size_t)n * n * (n / 2 + 1)); }
+
+bool config_ok(const fpm_config* c) {
+  if (!c) return false;
+  if (!fft_size_supported(c->ng) || !fft_size_supported(c->np)) return false;
+  if (c->np > c->ng || c->ng % c->np != 0) return false;
+  if (!(c->omega_m > 0.0 && c->omega_m <= 1.0)) return false;
+  if (c->kernel_mode < FPM_KERNEL_PAPER || c->kernel_mode > FPM_KERNEL_MIXED) return false;
+  if (c->factor_mode < FPM_FACTORS_FASTPM || c->factor_mode > FPM_FACTORS_QUINN) return false;
+  if (c->force_path < FPM_FORCE_UNFUSED || c->force_path > FPM_FORCE_FUSED) return false;
+  if (c->reserved != 0) return false;
+  return true;
+}
+
+// carved views of the caller's workspace
+struct Workspace {
+  float* rho;
+  float2* dk;
+  float2* fk[3];
+  float* F[3];
+};
+
+Workspace carve(const fpm_ctx* ctx) {
+  Workspace w;
+  char* p = static_cast<char*>(ctx->ws);
+  const int n = ctx->cfg.ng;
+  w.rho = reinterpret_cast<float*>(p); p += real_bytes(n);
+  for (int d = 0; d < 3; ++d) { w.F[d] = reinterpret_cast<float*>(p); p += real_bytes(n); }
+  w.dk = reinterpret_cast<float2*>(p); p += cplx_bytes(n);
+  for (int d = 0; d < 3; ++d) { w.fk[d] = reinterpret_cast<float2*>(p); p += cplx_bytes(n); }
+  return w;
+}
+
+int fail(fpm_ctx* ctx, int code, const char* what) {
+  if (ctx) {
+    ctx->err = what;
+    if (code == FPM_ECUDA) ctx->sticky = true;
+  }
+  return code;
+}
+
+int cuda_fail(fpm_ctx* ctx, cudaError_t e, const char* where) {
+  char buf[256];
+  std::snprintf(buf, sizeof buf, "%s: %s", where, cudaGetErrorString(e));
+  return fail(ctx, FPM_ECUDA, buf);
+}
+
+#define FPM_ENTER(ctx)                                              \
+  if (!(ctx)) return FPM_EINVAL;                                    \
+  if ((ctx)->sticky) return FPM_ECUDA;
+#define FPM_CUDA(ctx, call)                                         \
+  do {                                                              \
+    cudaError_t e__ = (call);                                       \
+    if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #call);    \
+  } while (0)
+#define FPM_REQUIRE(ctx, cond, what)                                \
+  if (!(cond)) return fail((ctx), FPM_EINVAL, what);
+#define FPM_NEED_WS(ctx)                                            \
+  if (!(ctx)->ws || (ctx)->ws_bytes < fpm_workspace_bytes(&(ctx)->cfg)) \
+    return fail((ctx), FPM_ENOMEM, "workspace missing or too small (fpm_set_workspace)");
+
+inline float particle_mass(const fpm_ctx* ctx) {
+  const float b = (float)(ctx->cfg.ng / ctx->cfg.np);
+  return b * b * b;
+}
+
+// paint -> r2c -> transfer function -> 3x c2r : the three force meshes of Alg. 3 ForceGrids(local)
+int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n) {
+  const int ng = ctx->cfg.ng;
+  cudaStream_t s = ctx->stream;
+  FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, s));
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s));
+  FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, w.dk, (float)(1.5 * ctx->cfg.omega_m), w.fk[0], w.fk[1],
+                                   w.fk[2], s));
+  for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.fk[d], w.F[d], s));
+  return FPM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* fpm_version(void) { return "fpm-b200 0.1 (sm_100a)"; }
+
+size_t fpm_workspace_bytes(const fpm_config* cfg) {
+  if (!config_ok(cfg)) return 0;
+  return 4 * real_bytes(cfg->ng) + 4 * cplx_bytes(cfg->ng);
+}
+
+int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
+  if (!out) return FPM_EINVAL;
+  *out = nullptr;
+  if (!config_ok(cfg)) return FPM_EINVAL;
+  fpm_ctx* ctx = new (std::nothrow) fpm_ctx();
+  if (!ctx) return FPM_ENOMEM;
+  ctx->cfg = *cfg;
+  ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t e = fft_tables_create(cfg->ng, &ctx->fft_g);
+  if (e == cudaSuccess) e = fft_tables_create(cfg->np, &ctx->fft_p);
+  if (e == cudaSuccess) e = kernel_tables_create(cfg->ng, cfg->kernel_mode, &ctx->kt_g);
+  if (e == cudaSuccess) e = kernel_tables_create(cfg->np, FPM_KERNEL_NAIVE, &ctx->kt_p);
+  if (e != cudaSuccess) {
+    fpm_destroy(ctx);
+    return FPM_ECUDA;
+  }
+  *out = ctx;
+  return FPM_OK;
+}
+
+int fpm_destroy(fpm_ctx* ctx) {
+  if (!ctx) return FPM_EINVAL;
+  fft_tables_destroy(&ctx->fft_g);
+  fft_tables_destroy(&ctx->fft_p);
+  kernel_tables_destroy(&ctx->kt_g);
+  kernel_tables_destroy(&ctx->kt_p);
+  delete ctx;
+  return FPM_OK;
+}
+
+const char* fpm_last_error(const fpm_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, ws != nullptr, "workspace is null");
+  FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(ws) & 255) == 0, "workspace must be 256-byte aligned");
+  if (bytes < fpm_workspace_bytes(&ctx->cfg)) return fail(ctx, FPM_ENOMEM, "workspace too small");
+  ctx->ws = ws;
+  ctx->ws_bytes = bytes;
+  return FPM_OK;
+}
+
+int fpm_growth(const fpm_ctx* ctx, double a, double* out) {
+  if (!ctx || !out || !(a > 0.0)) return FPM_EINVAL;
+  const GrowthOut g = growth(ctx->cfg.omega_m, a);
+  out[0] = g.D1; out[1] = g.f1; out[2] = g.D2; out[3] = g.f2; out[4] = g.E; out[5] = g.Gf; out[6] = g.gf;
+  return FPM_OK;
+}
+
+int fpm_drift_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out) {
+  if (!ctx || !out || !(ai > 0.0 && ac > 0.0 && af > 0.0)) return FPM_EINVAL;
+  *out = drift_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  return FPM_OK;
+}
+
+int fpm_kick_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out) {
+  if (!ctx || !out || !(ai > 0.0 && ac > 0.0 && af > 0.0)) return FPM_EINVAL;
+  *out = kick_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  return FPM_OK;
+}
+
+int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, float* mesh) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && mesh && (pos || n == 0), "fpm_paint: bad arguments");
+  FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, real && cplx, "fpm_fft_r2c: null pointer");
+  FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
+              "fpm_fft_r2c: pointers must be 8-byte aligned");
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, real, reinterpret_cast<float2*>(cplx), ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, real && cplx, "fpm_fft_c2r: null pointer");
+  FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
+              "fpm_fft_c2r: pointers must be 8-byte aligned");
+  FPM_CUDA(ctx, fft_c2r(ctx->fft_g, reinterpret_cast<float2*>(cplx), real, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, float* fkx, float* fky,
+                           float* fkz) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, delta_k && fkx && fky && fkz, "fpm_apply_force_kernel: null pointer");
+  FPM_REQUIRE(ctx, delta_k != fkx && delta_k != fky && delta_k != fkz,
+              "fpm_apply_force_kernel: outputs must not alias the input");
+  FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, reinterpret_cast<const float2*>(delta_k), scale,
+                                   reinterpret_cast<float2*>(fkx), reinterpret_cast<float2*>(fky),
+                                   reinterpret_cast<float2*>(fkz), ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, float* out) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && mesh && ((pos && out) || n == 0), "fpm_readout: bad arguments");
+  FPM_CUDA(ctx, readout(mesh, pos, n, ctx->cfg.ng, out, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_force(fpm_ctx* ctx, const float* pos, int64_t n, float* force) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((pos && force) || n == 0), "fpm_force: bad arguments");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  const int rc = force_meshes(ctx, w, pos, n);
+  if (rc != FPM_OK) return rc;
+  FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ctx->cfg.ng, force, ctx->stream));
+  return FPM_OK;
+}
+
+const float* fpm_workspace_density(const fpm_ctx* ctx) {
+  if (!ctx || !ctx->ws) return nullptr;
+  return carve(ctx).rho;
+}
+
+int fpm_kick(fpm_ctx* ctx, float* mom, const float* force, int64_t n, double ai, double ac,
+             double af) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((mom && force) || n == 0), "fpm_kick: bad arguments");
+  FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_kick: scale factors must be positive");
+  const double k = kick_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  FPM_CUDA(ctx, kick(mom, force, 3 * n, (float)k, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_drift(fpm_ctx* ctx, float* pos, const float* mom, int64_t n, double ai, double ac,
+              double af) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((pos && mom) || n == 0), "fpm_drift: bad arguments");
+  FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_drift: scale factors must be positive");
+  const double d = drift_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  FPM_CUDA(ctx, drift(pos, mom, 3 * n, (float)d, ctx->cfg.ng, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, float* pos,
+                 float* mom) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, delta_lin && pos && mom, "fpm_lpt_init: null pointer");
+  FPM_REQUIRE(ctx, order == 1 || order == 2, "fpm_lpt_init: order must be 1 or 2");
+  FPM_REQUIRE(ctx, a0 > 0.0, "fpm_lpt_init: a0 must be positive");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  cudaStream_t s = ctx->stream;
+  const int np = ctx->cfg.np, ng = ctx->cfg.ng, bfac = ng / np;
+  const int64_t n3 = (int64_t)np * np * np;
+  const GrowthOut g = growth(ctx->cfg.omega_m, a0);
+  const double pre = a0 * a0 * g.E;
+  float2 *dk = w.dk, *tk = w.fk[0], *sk = w.fk[1];
+  float *ra = w.F[0], *rb = w.F[1], *rc = w.F[2], *src = w.rho;
+
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_p, delta_lin, dk, s));
+  // psi1_d = c2r(i k_d delta / k^2);  x = q + D1 psi1,  p = a^2 E f1 D1 psi1   (1LPT / Zel'dovich)
+  for (int d = 0; d < 3; ++d) {
+    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, d, -1, -1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
+    FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D1, (float)(pre * g.f1 * g.D1), true,
+                               pos + d * n3, mom + d * n3, s));
+  }
+  if (order == 2) {
+    // S = sum_{i<j} (phi,ii phi,jj - phi,ij^2), phi,ij = c2r(k_i k_j delta / k^2)
+    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 0, 0, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
+    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 1, 1, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rb, s));
+    FPM_CUDA(ctx, lpt_source(src, ra, rb, nullptr, n3, 0, s));
+    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 2, 2, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rc, s));
+    FPM_CUDA(ctx, lpt_source(src, ra, rb, rc, n3, 1, s));
+    const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+    for (auto& pr : pairs) {
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, pr[0], pr[1], 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
+      FPM_CUDA(ctx, lpt_source(src, ra, nullptr, nullptr, n3, 2, s));
+    }
+    FPM_CUDA(ctx, fft_r2c(ctx->fft_p, src, sk, s));
+    // psi2_d = c2r(-i k_d S / k^2);  x += D2 psi2,  p += a^2 E f2 D2 psi2
+    for (int d = 0; d < 3; ++d) {
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, sk, tk, d, -1, 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
+      FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D2, (float)(pre * g.f2 * g.D2), false,
+                                 pos + d * n3, mom + d * n3, s));
+    }
+  }
+  FPM_CUDA(ctx, lpt_wrap(pos, 3 * n3, ng, s));
+  return FPM_OK;
+}
+
+int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int n_steps,
+              float* traj) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, pos && mom && a_stages && n_steps >= 0, "fpm_nbody: bad arguments");
+  for (int j = 0; j <= n_steps; ++j)
+    FPM_REQUIRE(ctx, a_stages[j] > 0.0, "fpm_nbody: scale factors must be positive");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  cudaStream_t s = ctx->stream;
+  const int ng = ctx->cfg.ng, np = ctx->cfg.np;
+  const int64_t n = (int64_t)np * np * np;
+  const double om = ctx->cfg.omega_m;
+  const int fm = ctx->cfg.factor_mode;
+
+  int rc = force_meshes(ctx, w, pos, n);
+  if (rc != FPM_OK) return rc;
+  if (traj) FPM_CUDA(ctx, cudaMemcpyAsync(traj, pos, sizeof(float) * 3 * n, cudaMemcpyDeviceToDevice, s));
+  double pending_kick = 0.0;   // second half kick of the previous step, same force mesh
+  for (int j = 0; j < n_steps; ++j) {
+    const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
+    const double k1 = kick_factor(om, ai, ai, ah, fm);
+    const double dr = drift_factor(om, ai, ah, af, fm);
+    FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ng,
+                                     (float)(pending_kick + k1), (float)dr, s));
+    rc = force_meshes(ctx, w, pos, n);
+    if (rc != FPM_OK) return rc;
+    if (traj)
+      FPM_CUDA(ctx, cudaMemcpyAsync(traj + (int64_t)(j + 1) * 3 * n, pos, sizeof(float) * 3 * n,
+                                    cudaMemcpyDeviceToDevice, s));
+    pending_kick = kick_factor(om, ah, af, af, fm);
+  }
+  if (n_steps > 0)
+    FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ng, (float)pending_kick, 0.f, s));
+  return FPM_OK;
+}
+
+int fpm_nbody_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom,
+                   const double* a_stages, int n_steps) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, h_pos && h_mom && d_pos && d_mom, "fpm_nbody_host: null pointer");
+  const int64_t n = (int64_t)ctx->cfg.np * ctx->cfg.np * ctx->cfg.np;
+  const size_t bytes = sizeof(float) * 3 * (size_t)n;
+  cudaStream_t s = ctx->stream;
+  FPM_CUDA(ctx, cudaMemcpyAsync(d_pos, h_pos, bytes, cudaMemcpyHostToDevice, s));
+  FPM_CUDA(ctx, cudaMemcpyAsync(d_mom, h_mom, bytes, cudaMemcpyHostToDevice, s));
+  const int rc = fpm_nbody(ctx, d_pos, d_mom, a_stages, n_steps, nullptr);
+  if (rc != FPM_OK) return rc;
+  FPM_CUDA(ctx, cudaMemcpyAsync(h_pos, d_pos, bytes, cudaMemcpyDeviceToHost, s));
+  FPM_CUDA(ctx, cudaMemcpyAsync(h_mom, d_mom, bytes, cudaMemcpyDeviceToHost, s));
+  FPM_CUDA(ctx, cudaStreamSynchronize(s));
+  return FPM_OK;
+}
+
+int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n,
+                      const float* grad_mesh, float* grad_pos, float* grad_mass) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_pos) || n == 0), "fpm_paint_adjoint: bad arguments");
+  FPM_CUDA(ctx, readout_grad(grad_mesh, pos, mass, particle_mass(ctx), n, ctx->cfg.ng, grad_pos,
+                             grad_mass, ctx->stream));
+  return FPM_OK;
+}
+
+int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n,
+                        const float* grad_out, float* grad_mesh, float* grad_pos) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_out) || n == 0), "fpm_readout_adjoint: bad arguments");
+  FPM_REQUIRE(ctx, !grad_pos || mesh, "fpm_readout_adjoint: grad_pos needs the forward mesh");
+  FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, ctx->stream));
+  if (grad_pos)
+    FPM_CUDA(ctx, readout_grad(mesh, pos, grad_out, 0.f, n, ctx->cfg.ng, grad_pos, nullptr, ctx->stream));
+  return FPM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,157 @@
+// fft.cu -- plan tables and launchers of the 3-D r2c / c2r transforms.
+// Forward order z (r2c) -> y -> x; inverse x -> y -> z (c2r).  The y and x passes are in place
+// on the half-complex buffer.  No cuFFT anywhere in this library.
+#include <cmath>
+#include <vector>
+
+#include "fft_kernels.cuh"
+#include "fpm_internal.h"
+
+namespace fpm {
+
+namespace {
+
+const double kPi = 3.14159265358979323846264338327950288;
+
+PlanInfo plan_info(int n) {
+  switch (n) {
+    case 4: return Plan<4>::info();
+    case 8: return Plan<8>::info();
+    case 16: return Plan<16>::info();
+    case 32: return Plan<32>::info();
+    case 64: return Plan<64>::info();
+    case 128: return Plan<128>::info();
+    case 256: return Plan<256>::info();
+    case 512: return Plan<512>::info();
+    case 1024: return Plan<1024>::info();
+    default: return PlanInfo{0, 0, 0, {0, 0, 0}};
+  }
+}
+
+// stage s >= 1: table[(t-1) NS + k] = exp(-2 pi i t k / (NS R_s)), t = 1..R_s-1, k < NS
+void build_stage_table(int n, std::vector<float2>& out) {
+  const PlanInfo pi = plan_info(n);
+  int ns = pi.r[0];
+  for (int s = 1; s < pi.nst; ++s) {
+    const int r = pi.r[s];
+    for (int t = 1; t < r; ++t)
+      for (int k = 0; k < ns; ++k) {
+        const double ang = -2.0 * kPi * (double)t * k / ((double)ns * r);
+        out.push_back(make_float2((float)std::cos(ang), (float)std::sin(ang)));
+      }
+    ns *= r;
+  }
+}
+
+template <class K>
+cudaError_t set_smem(K kernel, size_t bytes) {
+  if (bytes <= 48 * 1024) return cudaSuccess;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <int N, bool INV>
+cudaError_t launch_cols(const float2* in, float2* out, int batches, int64_t batch_stride, int ncols,
+                        int64_t line_stride, const float2* tw, cudaStream_t s) {
+  constexpr int T = col_tile<N>();
+  constexpr int threads = T * Plan<N>::P;
+  const size_t smem = Plan<N>::NST > 1 ? sizeof(float2) * N * T : 0;
+  auto kern = fft_cols_kernel<N, INV, OpNone, OpNone>;
+  cudaError_t e = set_smem(kern, smem);
+  if (e != cudaSuccess) return e;
+  dim3 grid((ncols + T - 1) / T, batches);
+  kern<<<grid, threads, smem, s>>>(in, out, batch_stride, ncols, line_stride, tw, OpNone{}, OpNone{});
+  return cudaGetLastError();
+}
+
+template <int N>
+cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaStream_t s) {
+  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
+  const int64_t nrows = (int64_t)N * N;
+  {
+    constexpr int threads = G * Plan<M>::P;
+    const size_t smem = sizeof(float2) * G * row_pitch(M);
+    auto kern = fft_z_r2c_kernel<N>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(real, cplx, nrows, t.stage_m, t.full);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  // y: one batch per x slab, columns kz, lines y (stride nzh)
+  cudaError_t e = launch_cols<N, false>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  if (e != cudaSuccess) return e;
+  // x: columns (y, kz) flattened, lines x (stride N nzh)
+  return launch_cols<N, false>(cplx, cplx, 1, 0, N * nzh, (int64_t)N * nzh, t.stage_n, s);
+}
+
+template <int N>
+cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t s) {
+  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
+  const int64_t nrows = (int64_t)N * N;
+  cudaError_t e = launch_cols<N, true>(cplx, cplx, 1, 0, N * nzh, (int64_t)N * nzh, t.stage_n, s);
+  if (e != cudaSuccess) return e;
+  e = launch_cols<N, true>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  if (e != cudaSuccess) return e;
+  constexpr int threads = G * Plan<M>::P;
+  const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
+  auto kern = fft_z_c2r_kernel<N>;
+  e = set_smem(kern, smem);
+  if (e != cudaSuccess) return e;
+  const float scale = (float)(1.0 / ((double)N * N * N));
+  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+bool fft_size_supported(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
+
+cudaError_t fft_tables_create(int n, FftTables* out) {
+  std::vector<float2> host;
+  build_stage_table(n, host);
+  const size_t off_m = host.size();
+  build_stage_table(n / 2, host);
+  const size_t off_f = host.size();
+  for (int k = 0; k < n / 2; ++k) {
+    const double ang = -2.0 * kPi * k / n;
+    host.push_back(make_float2((float)std::cos(ang), (float)std::sin(ang)));
+  }
+  float2* dev = nullptr;
+  cudaError_t e = cudaMalloc(&dev, host.size() * sizeof(float2));
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(dev, host.data(), host.size() * sizeof(float2), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(dev); return e; }
+  out->n = n;
+  out->dev = dev;
+  out->stage_n = dev;
+  out->stage_m = dev + off_m;
+  out->full = dev + off_f;
+  return cudaSuccess;
+}
+
+void fft_tables_destroy(FftTables* t) {
+  if (t->dev) cudaFree(t->dev);
+  *t = FftTables{};
+}
+
+#define FPM_FFT_DISPATCH(fn, ...)                        \
+  switch (t.n) {                                         \
+    case 8: return fn<8>(__VA_ARGS__);                   \
+    case 16: return fn<16>(__VA_ARGS__);                 \
+    case 32: return fn<32>(__VA_ARGS__);                 \
+    case 64: return fn<64>(__VA_ARGS__);                 \
+    case 128: return fn<128>(__VA_ARGS__);               \
+    case 256: return fn<256>(__VA_ARGS__);               \
+    case 512: return fn<512>(__VA_ARGS__);               \
+    case 1024: return fn<1024>(__VA_ARGS__);             \
+    default: return cudaErrorInvalidValue;               \
+  }
+
+cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s) {
+  FPM_FFT_DISPATCH(r2c_impl, t, real, cplx, s)
+}
+cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s) {
+  FPM_FFT_DISPATCH(c2r_impl, t, cplx, real, s)
+}
+
+}  // namespace fpm

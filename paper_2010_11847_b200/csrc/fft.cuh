@@ -1,0 +1,192 @@
+// fft.cuh -- hand-written batched 1-D FFT passes for the 3-D r2c / c2r transforms of the PM step
+// ("one forward 3D FFT ... three inverse FFTs"; Alg. 3 FFT3D / iFFT3D,
+// PAPER.md:283-290).  sm_100a design notes:
+//   * the transform is HBM-bound (2.8 flop/B), so each axis is exactly one read + one write of
+//     the mesh; a thread keeps E = 8..32 complex points in registers, which gives every SM
+//     >100 KB of loads in flight with few resident warps;
+//   * Stockham autosort stages of radix <= 32 in registers; stages exchange through shared
+//     memory once (N <= 1024 needs at most 2 stages); first-stage loads and last-stage stores
+//     go straight between HBM and registers;
+//   * strided axes (y, x) are processed as tiles of T contiguous columns so that every global
+//     access is a >=128-byte segment and shared memory is conflict-free by construction;
+//   * inverse transforms run the forward butterflies on (im, re)-swapped data;
+//   * inter-stage twiddles come from small per-stage tables laid out [t][k] (coalesced, L1
+//     resident, correctly rounded from float64) -- no sincosf in the loop.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <utility>
+
+namespace fpm {
+
+// ------------------------------------------------------------------------------------------
+// complex helpers
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cswap(float2 a) { return make_float2(a.y, a.x); }
+
+// cos(2 pi k / 32), k = 0..8
+__host__ __device__ constexpr float cos32_table(int k) {
+  constexpr float c[9] = {1.0f,
+                          0.98078528040323044913f,
+                          0.92387953251128675613f,
+                          0.83146961230254523708f,
+                          0.70710678118654752440f,
+                          0.55557023301960222474f,
+                          0.38268343236508977173f,
+                          0.19509032201612826785f,
+                          0.0f};
+  return c[k];
+}
+__host__ __device__ constexpr float cos32(int k) {
+  k = ((k % 32) + 32) % 32;
+  if (k > 16) k = 32 - k;
+  return k > 8 ? -cos32_table(16 - k) : cos32_table(k);
+}
+__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+
+// x * exp(-2 pi i I / R), resolved at compile time
+template <int R, int I>
+__device__ __forceinline__ float2 mul_twiddle(float2 x) {
+  constexpr int k = (I * (32 / R)) % 32;
+  if constexpr (k == 0) return x;
+  else if constexpr (k == 8) return make_float2(x.y, -x.x);
+  else if constexpr (k == 16) return make_float2(-x.x, -x.y);
+  else if constexpr (k == 24) return make_float2(-x.y, x.x);
+  else {
+    constexpr float c = cos32(k), s = -sin32(k);
+    return make_float2(x.x * c - x.y * s, x.x * s + x.y * c);
+  }
+}
+
+// In-register forward DFT of R points (decimation in frequency), natural-order output.
+template <int R>
+struct Dft {
+  template <int... I>
+  static __device__ __forceinline__ void run(float2 (&v)[R], std::integer_sequence<int, I...>) {
+    float2 e[R / 2], o[R / 2];
+    ((e[I] = cadd(v[I], v[I + R / 2]), o[I] = mul_twiddle<R, I>(csub(v[I], v[I + R / 2]))), ...);
+    Dft<R / 2>::apply(e);
+    Dft<R / 2>::apply(o);
+    ((v[2 * I] = e[I], v[2 * I + 1] = o[I]), ...);
+  }
+  static __device__ __forceinline__ void apply(float2 (&v)[R]) {
+    run(v, std::make_integer_sequence<int, R / 2>{});
+  }
+};
+template <>
+struct Dft<1> {
+  static __device__ __forceinline__ void apply(float2 (&)[1]) {}
+};
+template <>
+struct Dft<2> {
+  static __device__ __forceinline__ void apply(float2 (&v)[2]) {
+    const float2 a = v[0], b = v[1];
+    v[0] = cadd(a, b);
+    v[1] = csub(a, b);
+  }
+};
+
+// ------------------------------------------------------------------------------------------
+// Plans: N = R0 * R1 * R2, every radix <= E (points held per thread), P = N / E threads per line.
+// ------------------------------------------------------------------------------------------
+struct PlanInfo {
+  int n, e, nst, r[3];
+};
+
+template <int N> struct Plan;
+#define FPM_PLAN(N_, E_, NST_, R0_, R1_, R2_)                                        \
+  template <> struct Plan<N_> {                                                      \
+    static constexpr int E = E_, NST = NST_, R0 = R0_, R1 = R1_, R2 = R2_;           \
+    static constexpr int P = N_ / E_;                                                \
+    __host__ __device__ static constexpr int radix(int s) { return s == 0 ? R0_ : (s == 1 ? R1_ : R2_); } \
+    /* number of lines already combined before stage s */                            \
+    __host__ __device__ static constexpr int ns(int s) { return s == 0 ? 1 : (s == 1 ? R0_ : R0_ * R1_); } \
+    /* offset of stage s (>= 1) in the twiddle table */                              \
+    __host__ __device__ static constexpr int toff(int s) { return s <= 1 ? 0 : (R1_ - 1) * R0_; } \
+    static constexpr int table_len = (NST_ > 1 ? (R1_ - 1) * R0_ : 0) + (NST_ > 2 ? (R2_ - 1) * R0_ * R1_ : 0); \
+    static constexpr PlanInfo info() { return PlanInfo{N_, E_, NST_, {R0_, R1_, R2_}}; } \
+  };
+FPM_PLAN(4, 4, 1, 4, 1, 1)
+FPM_PLAN(8, 8, 1, 8, 1, 1)
+FPM_PLAN(16, 16, 1, 16, 1, 1)
+FPM_PLAN(32, 8, 2, 8, 4, 1)
+FPM_PLAN(64, 8, 2, 8, 8, 1)
+FPM_PLAN(128, 16, 2, 16, 8, 1)
+FPM_PLAN(256, 16, 2, 16, 16, 1)
+FPM_PLAN(512, 32, 2, 32, 16, 1)
+FPM_PLAN(1024, 32, 2, 32, 32, 1)
+#undef FPM_PLAN
+
+// shared-memory accessors -----------------------------------------------------------------
+// column tile: element i of column c at i*T + c (lanes run over c: conflict-free)
+template <int T>
+struct ColSmem {
+  float2* base;
+  int c;
+  __device__ __forceinline__ void st(int i, float2 x) const { base[i * T + c] = x; }
+  __device__ __forceinline__ float2 ld(int i) const { return base[i * T + c]; }
+};
+// contiguous line: lanes run over the butterfly index; one pad slot per 16 breaks stride-R conflicts
+struct RowSmem {
+  float2* row;
+  __device__ __forceinline__ void st(int i, float2 x) const { row[i + (i >> 4)] = x; }
+  __device__ __forceinline__ float2 ld(int i) const { return row[i + (i >> 4)]; }
+};
+__host__ __device__ constexpr int row_pitch(int m) { return m + (m >> 4) + 1; }
+
+// ------------------------------------------------------------------------------------------
+// One Stockham stage and the recursive driver.  Thread p of a line holds v[e] = x[p + P e].
+// Stage with radix R, NS lines already combined: butterfly j reads x[j + t N/R], multiplies by
+// exp(-2 pi i t k/(NS R)), k = j mod NS, and writes y[(j-k) R + k + t NS].
+// ------------------------------------------------------------------------------------------
+template <int N, int S, class SM>
+__device__ __forceinline__ void fft_stage(float2 (&v)[Plan<N>::E], const int p, const SM& sm,
+                                          const float2* __restrict__ tw) {
+  using PL = Plan<N>;
+  constexpr int E = PL::E, P = PL::P, R = PL::radix(S), NS = PL::ns(S), M = E / R;
+  constexpr bool last = (S == PL::NST - 1);
+#pragma unroll
+  for (int u = 0; u < M; ++u) {
+    const int j = p + u * P;
+    const int k = j & (NS - 1);
+    float2 a[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) a[t] = v[u + t * M];
+    if constexpr (NS > 1) {
+      const float2* __restrict__ tws = tw + PL::toff(S) + k;
+#pragma unroll
+      for (int t = 1; t < R; ++t) a[t] = cmul(a[t], __ldg(tws + (t - 1) * NS));
+    }
+    Dft<R>::apply(a);
+    if constexpr (last) {
+#pragma unroll
+      for (int t = 0; t < R; ++t) v[u + t * M] = a[t];
+    } else {
+      const int base = (j - k) * R + k;
+#pragma unroll
+      for (int t = 0; t < R; ++t) sm.st(base + t * NS, a[t]);
+    }
+  }
+  if constexpr (!last) {
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = sm.ld(p + P * e);
+    if constexpr (S + 1 < PL::NST - 1) __syncthreads();
+    fft_stage<N, S + 1, SM>(v, p, sm, tw);
+  }
+}
+
+// forward DFT of one line: in v[e] = x[p + P e], out v[e] = X[p + P e]
+template <int N, class SM>
+__device__ __forceinline__ void fft_line(float2 (&v)[Plan<N>::E], const int p, const SM& sm,
+                                         const float2* __restrict__ tw) {
+  fft_stage<N, 0, SM>(v, p, sm, tw);
+}
+
+}  // namespace fpm

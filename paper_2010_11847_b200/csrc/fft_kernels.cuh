@@ -1,0 +1,141 @@
+// fft_kernels.cuh -- the three pass kernels of the 3-D transform (see fft.cuh for the design).
+//   fft_z_r2c_kernel : contiguous axis, real -> half-complex, N/2-point complex FFT + split
+//   fft_cols_kernel  : strided axes (y then x forward; x then y inverse), in place, tile of T columns,
+//                      with optional element-wise LoadOp/StoreOp (the fused Green's function,
+//                      PAPER.md:49-59, rides on the x pass)
+//   fft_z_c2r_kernel : contiguous axis, half-complex -> real, merge + N/2-point inverse FFT
+#pragma once
+#include "fft.cuh"
+
+namespace fpm {
+
+struct OpNone {
+  // v: value, line: index along the transformed axis, col: column index inside the batch
+  __device__ __forceinline__ float2 load(float2 v, int, int64_t, int) const { return v; }
+  __device__ __forceinline__ float2 store(float2 v, int, int64_t, int) const { return v; }
+};
+
+template <int N> __host__ __device__ constexpr int col_tile() { return N >= 64 ? 16 : 32; }
+template <int N> __host__ __device__ constexpr int z_rows() {          // lines per block on the z pass
+  constexpr int P = Plan<N / 2>::P;
+  return P >= 256 ? 1 : 256 / P;
+}
+
+// in/out may alias (in place): each block reads its whole tile before writing it.
+// grid = (ceil(ncols / T), batches); element (line i, column c) of batch b at
+//   b * batch_stride + i * line_stride + c.
+template <int N, bool INV, class LOADOP, class STOREOP>
+__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
+                int64_t line_stride, const float2* __restrict__ tw, LOADOP lop, STOREOP sop) {
+  extern __shared__ float2 smem[];
+  using PL = Plan<N>;
+  constexpr int T = col_tile<N>(), E = PL::E, P = PL::P;
+  const int c = threadIdx.x % T, p = threadIdx.x / T;
+  const int64_t col = (int64_t)blockIdx.x * T + c;
+  const bool ok = col < ncols;
+  const int64_t off = (int64_t)blockIdx.y * batch_stride + col;
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    float2 x = make_float2(0.f, 0.f);
+    if (ok) x = lop.load(in[off + (int64_t)i * line_stride], i, col, blockIdx.y);
+    v[e] = INV ? cswap(x) : x;
+  }
+  ColSmem<T> sm{smem, c};
+  fft_line<N>(v, p, sm, tw);
+  if (ok) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int i = p + P * e;
+      const float2 x = INV ? cswap(v[e]) : v[e];
+      out[off + (int64_t)i * line_stride] = sop.store(x, i, col, blockIdx.y);
+    }
+  }
+}
+
+// real rows of N floats -> rows of N/2+1 complex.  twn[k] = exp(-2 pi i k / N), k < N/2.
+template <int N>
+__global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
+fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t nrows,
+                 const float2* __restrict__ tw, const float2* __restrict__ twn) {
+  extern __shared__ float2 smem[];
+  constexpr int M = N / 2;
+  using PL = Plan<M>;
+  constexpr int E = PL::E, P = PL::P, G = z_rows<N>();
+  const int p = threadIdx.x % P, g = threadIdx.x / P;
+  const int64_t row = (int64_t)blockIdx.x * G + g;
+  const bool ok = row < nrows;
+  const float2* src = reinterpret_cast<const float2*>(in) + row * M;
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) v[e] = ok ? src[p + P * e] : make_float2(0.f, 0.f);
+  RowSmem sm{smem + g * row_pitch(M)};
+  fft_line<M>(v, p, sm, tw);
+  if constexpr (PL::NST > 1) __syncthreads();
+#pragma unroll
+  for (int e = 0; e < E; ++e) sm.st(p + P * e, v[e]);
+  __syncthreads();
+  if (!ok) return;
+  float2* dst = out + row * (M + 1);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int k = p + P * e;
+    const float2 zk = v[e];
+    if (k == 0) {
+      dst[0] = make_float2(zk.x + zk.y, 0.f);
+      dst[M] = make_float2(zk.x - zk.y, 0.f);
+    } else {
+      const float2 zm = sm.ld(M - k);
+      // Xe = (Z[k] + conj Z[M-k])/2, Xo = (Z[k] - conj Z[M-k])/(2i), X[k] = Xe + W_N^k Xo
+      const float2 xe = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+      const float2 d = make_float2(0.5f * (zk.x - zm.x), 0.5f * (zk.y + zm.y));
+      const float2 xo = make_float2(d.y, -d.x);
+      dst[k] = cadd(xe, cmul(__ldg(twn + k), xo));
+    }
+  }
+}
+
+// rows of N/2+1 complex -> real rows of N floats, times `scale`.
+template <int N>
+__global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
+fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t nrows,
+                 const float2* __restrict__ tw, const float2* __restrict__ twn, float scale) {
+  extern __shared__ float2 smem[];
+  constexpr int M = N / 2;
+  using PL = Plan<M>;
+  constexpr int E = PL::E, P = PL::P, G = z_rows<N>();
+  const int p = threadIdx.x % P, g = threadIdx.x / P;
+  const int64_t row = (int64_t)blockIdx.x * G + g;
+  const bool ok = row < nrows;
+  const float2* src = in + row * (M + 1);
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int k = p + P * e;
+    float2 z = make_float2(0.f, 0.f);
+    if (ok) {
+      const float2 xk = src[k], xm = src[M - k];
+      if (k == 0) {
+        z = make_float2(xk.x + xm.x, xk.x - xm.x);
+      } else {
+        // A = X[k] + conj X[M-k], B = (X[k] - conj X[M-k]) exp(+2 pi i k/N), Z = A + i B
+        const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
+        const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
+        const float2 w = __ldg(twn + k);
+        const float2 b = cmul(d, make_float2(w.x, -w.y));
+        z = make_float2(a.x - b.y, a.y + b.x);
+      }
+    }
+    v[e] = cswap(z);
+  }
+  RowSmem sm{smem + g * row_pitch(M)};
+  fft_line<M>(v, p, sm, tw);
+  if (!ok) return;
+  float2* dst = reinterpret_cast<float2*>(out) + row * M;
+#pragma unroll
+  for (int e = 0; e < E; ++e) dst[p + P * e] = make_float2(v[e].y * scale, v[e].x * scale);
+}
+
+}  // namespace fpm

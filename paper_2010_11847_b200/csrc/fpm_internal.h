@@ -1,0 +1,91 @@
+// fpm_internal.h -- context and internal launch interfaces of libfpm (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/fpm.h"
+
+namespace fpm {
+
+// ---- FFT (fft.cu) ---------------------------------------------------------------------------
+struct FftTables {
+  int n = 0;
+  float2* dev = nullptr;       // one allocation: [stage table N][stage table N/2][W_N^k, k < N/2]
+  float2* stage_n = nullptr;
+  float2* stage_m = nullptr;
+  float2* full = nullptr;
+};
+cudaError_t fft_tables_create(int n, FftTables* out);
+void fft_tables_destroy(FftTables* t);
+bool fft_size_supported(int n);
+
+// per-axis tables of the transfer function, fp32 rounded from float64 (green.cu)
+struct KernelTables {
+  int n = 0;
+  float* dev = nullptr;
+  float* lap = nullptr;    // K^2 contribution of one axis: (2 sin(w/2))^2 or w^2
+  float* grad = nullptr;   // g(w) with the Nyquist entry zeroed
+  float* kvec = nullptr;   // w = 2 pi f / n (Nyquist kept)           [LPT spectral kernels]
+  float* kvec0 = nullptr;  // w with the Nyquist entry zeroed          [LPT spectral kernels]
+};
+cudaError_t kernel_tables_create(int n, int kernel_mode, KernelTables* out);
+void kernel_tables_destroy(KernelTables* t);
+
+// element-wise epilogue/prologue selectors for the fused x passes (fft.cu)
+enum XOp { XOP_NONE = 0, XOP_INVLAP = 1, XOP_GRAD = 2 };
+
+cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s);
+cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s);
+
+// ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
+cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
+                  float* mesh, bool zero_first, cudaStream_t s);
+cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, float* out,
+                    cudaStream_t s);
+cudaError_t readout3(const float* fx, const float* fy, const float* fz, const float* pos, int64_t n,
+                     int ng, float* out3, cudaStream_t s);
+// gradient of the CIC sum w.r.t. the position, times scale_p (mass[p] or vbar[p] or constant)
+cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale, float scale_const,
+                         int64_t n, int ng, float* out3, float* out_value, cudaStream_t s);
+
+// ---- particle updates (particles.cu) -----------------------------------------------------------
+cudaError_t kick(float* mom, const float* force, int64_t n3, float fac, cudaStream_t s);
+cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, cudaStream_t s);
+// mom += force(pos) * kfac ; pos = wrap(pos + mom * dfac), gathering the three force meshes
+cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
+                               float* mom, int64_t n, int ng, float kfac, float dfac,
+                               cudaStream_t s);
+
+// ---- transfer function and LPT element-wise kernels (green.cu) ---------------------------------
+cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float scale, float2* fkx,
+                               float2* fky, float2* fkz, cudaStream_t s);
+// out = mult(k) in, mult = sign * (a == b ? -k_a^2 : (i k_a)(b >= 0 ? i k_b : 1)) * (-1/k^2)
+cudaError_t lpt_spectral(const KernelTables& kt, const float2* in, float2* out, int a, int b,
+                         float sign, cudaStream_t s);
+cudaError_t lpt_displace(const float* psi, int np, int bfac, int axis, float dcoef, float vcoef,
+                         bool first, float* pos_d, float* mom_d, cudaStream_t s);
+cudaError_t lpt_wrap(float* pos, int64_t n3, int ng, cudaStream_t s);
+// s = a*b (mode 0), s += (a+b)*c (mode 1), s -= a*a (mode 2)
+cudaError_t lpt_source(float* s, const float* a, const float* b, const float* c, int64_t n, int mode,
+                       cudaStream_t st);
+
+// ---- background cosmology on the host, float64 (cosmology.cpp) ---------------------------------
+struct GrowthOut { double D1, f1, D2, f2, E, Gf, gf; };
+GrowthOut growth(double omega_m, double a);
+double drift_factor(double omega_m, double ai, double ac, double af, int factor_mode);
+double kick_factor(double omega_m, double ai, double ac, double af, int factor_mode);
+
+}  // namespace fpm
+
+struct fpm_ctx {
+  fpm_config cfg;
+  cudaStream_t stream = nullptr;
+  fpm::FftTables fft_g, fft_p;      // plans for ng and np (same object when equal)
+  fpm::KernelTables kt_g, kt_p;     // transfer-function tables on ng; spectral tables on np
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  bool sticky = false;
+  std::string err;
+};

@@ -1,0 +1,193 @@
+// green.cu -- the transfer function grad laplace^-1 in k-space (Eq. 3-5) as a
+// stand-alone element-wise kernel (the fused variants ride on the FFT x passes, fft.cu), and the
+// spectral element-wise kernels of the LPT initial conditions (Alg. 4).
+#include <cmath>
+#include <vector>
+
+#include "fpm_internal.h"
+
+namespace fpm {
+
+namespace {
+
+const double kPi = 3.14159265358979323846264338327950288;
+constexpr int kThreads = 128;
+
+// One block per (x, y) row of the half-complex mesh, threads over kz.
+__global__ void __launch_bounds__(kThreads)
+force_kernel_rows(const float2* __restrict__ dk, int n, const float* __restrict__ lap,
+                  const float* __restrict__ grad, float scale, float2* __restrict__ fkx,
+                  float2* __restrict__ fky, float2* __restrict__ fkz) {
+  const int nzh = n / 2 + 1;
+  const int x = blockIdx.x / n, y = blockIdx.x % n;
+  const float lxy = __ldg(lap + x) + __ldg(lap + y);
+  const float gx = __ldg(grad + x), gy = __ldg(grad + y);
+  const int64_t row = (int64_t)blockIdx.x * nzh;
+  for (int z = threadIdx.x; z < nzh; z += blockDim.x) {
+    const float k2 = lxy + __ldg(lap + z);
+    const float inv = (blockIdx.x == 0 && z == 0) ? 0.f : scale / k2;
+    const float2 d = dk[row + z];
+    // i g d / K^2 : (re, im) -> (-im, re) * g * inv
+    const float2 id = make_float2(-d.y * inv, d.x * inv);
+    const float gz = __ldg(grad + z);
+    fkx[row + z] = make_float2(id.x * gx, id.y * gx);
+    fky[row + z] = make_float2(id.x * gy, id.y * gy);
+    fkz[row + z] = make_float2(id.x * gz, id.y * gz);
+  }
+}
+
+// out = sign * mult(k) * (-1/k^2) * in ; mult = -k_a^2 (a == b), (i k_a)(i k_b) (a != b, b >= 0),
+// i k_a (b < 0); i k_d uses the Nyquist-zeroed table, -k_a^2 the full one.
+__global__ void __launch_bounds__(kThreads)
+lpt_spectral_rows(const float2* __restrict__ in, float2* __restrict__ out, int n,
+                  const float* __restrict__ kv, const float* __restrict__ kv0, int a, int b,
+                  float sign) {
+  const int nzh = n / 2 + 1;
+  const int x = blockIdx.x / n, y = blockIdx.x % n;
+  const int64_t row = (int64_t)blockIdx.x * nzh;
+  const float kx = __ldg(kv + x), ky = __ldg(kv + y);
+  for (int z = threadIdx.x; z < nzh; z += blockDim.x) {
+    const int idx[3] = {x, y, z};
+    const float kz = __ldg(kv + z);
+    const float k2 = kx * kx + ky * ky + kz * kz;
+    const float inv = (blockIdx.x == 0 && z == 0) ? 0.f : -sign / k2;
+    const float2 v = in[row + z];
+    float2 r;
+    if (a == b) {
+      const float ka = __ldg(kv + idx[a]);
+      const float m = -ka * ka * inv;
+      r = make_float2(v.x * m, v.y * m);
+    } else if (b >= 0) {
+      const float m = -__ldg(kv0 + idx[a]) * __ldg(kv0 + idx[b]) * inv;   // (i ka)(i kb) = -ka kb
+      r = make_float2(v.x * m, v.y * m);
+    } else {
+      const float m = __ldg(kv0 + idx[a]) * inv;                          // i ka
+      r = make_float2(-v.y * m, v.x * m);
+    }
+    out[row + z] = r;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+lpt_displace_kernel(const float* __restrict__ psi, int np, int bfac, int axis, float dcoef,
+                    float vcoef, int first, float* __restrict__ pos_d, float* __restrict__ mom_d) {
+  const int64_t n3 = (int64_t)np * np * np;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n3;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const float s = psi[i] * (float)bfac;
+    if (first) {
+      const int64_t q = axis == 0 ? i / ((int64_t)np * np) : (axis == 1 ? (i / np) % np : i % np);
+      pos_d[i] = (float)(q * bfac) + dcoef * s;
+      mom_d[i] = vcoef * s;
+    } else {
+      pos_d[i] += dcoef * s;
+      mom_d[i] += vcoef * s;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+lpt_wrap_kernel(float* __restrict__ pos, int64_t n, float ng, float inv_ng) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    float x = pos[i];
+    x -= ng * floorf(x * inv_ng);
+    if (x >= ng) x -= ng;
+    if (x < 0.f) x += ng;
+    pos[i] = x >= ng ? 0.f : x;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+lpt_source_kernel(float* __restrict__ s, const float* __restrict__ a, const float* __restrict__ b,
+                  const float* __restrict__ c, int64_t n, int mode) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    if (mode == 0) s[i] = a[i] * b[i];
+    else if (mode == 1) s[i] += (a[i] + b[i]) * c[i];
+    else s[i] -= a[i] * a[i];
+  }
+}
+
+inline unsigned grid_for(int64_t n) {
+  int64_t b = (n + 255) / 256;
+  if (b > 148LL * 32) b = 148LL * 32;
+  return (unsigned)(b < 1 ? 1 : b);
+}
+
+}  // namespace
+
+cudaError_t kernel_tables_create(int n, int kernel_mode, KernelTables* out) {
+  std::vector<float> host(4 * (size_t)n);
+  for (int i = 0; i < n; ++i) {
+    const int f = i <= n / 2 ? i : i - n;       // integer frequency in (-n/2, n/2]
+    const double w = 2.0 * kPi * f / n;
+    const bool nyq = (2 * f == n);
+    double lap, grad;
+    if (kernel_mode == FPM_KERNEL_PAPER) {
+      const double s = 2.0 * std::sin(0.5 * w);
+      lap = s * s;                                                // Eq. 4, (w sinc(w/2))^2
+    } else {
+      lap = w * w;
+    }
+    if (kernel_mode == FPM_KERNEL_NAIVE) grad = w;
+    else grad = (8.0 * std::sin(w) - std::sin(2.0 * w)) / 6.0;    // Eq. 5
+    if (nyq) grad = 0.0;
+    host[i] = (float)lap;
+    host[n + i] = (float)grad;
+    host[2 * n + i] = (float)w;
+    host[3 * n + i] = nyq ? 0.f : (float)w;
+  }
+  float* dev = nullptr;
+  cudaError_t e = cudaMalloc(&dev, host.size() * sizeof(float));
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(dev, host.data(), host.size() * sizeof(float), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(dev); return e; }
+  out->n = n;
+  out->dev = dev;
+  out->lap = dev;
+  out->grad = dev + n;
+  out->kvec = dev + 2 * n;
+  out->kvec0 = dev + 3 * n;
+  return cudaSuccess;
+}
+
+void kernel_tables_destroy(KernelTables* t) {
+  if (t->dev) cudaFree(t->dev);
+  *t = KernelTables{};
+}
+
+cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float scale, float2* fkx,
+                               float2* fky, float2* fkz, cudaStream_t s) {
+  force_kernel_rows<<<(unsigned)(kt.n * kt.n), kThreads, 0, s>>>(dk, kt.n, kt.lap, kt.grad, scale,
+                                                                fkx, fky, fkz);
+  return cudaGetLastError();
+}
+
+cudaError_t lpt_spectral(const KernelTables& kt, const float2* in, float2* out, int a, int b,
+                         float sign, cudaStream_t s) {
+  lpt_spectral_rows<<<(unsigned)(kt.n * kt.n), kThreads, 0, s>>>(in, out, kt.n, kt.kvec, kt.kvec0, a,
+                                                                b, sign);
+  return cudaGetLastError();
+}
+
+cudaError_t lpt_displace(const float* psi, int np, int bfac, int axis, float dcoef, float vcoef,
+                         bool first, float* pos_d, float* mom_d, cudaStream_t s) {
+  const int64_t n3 = (int64_t)np * np * np;
+  lpt_displace_kernel<<<grid_for(n3), 256, 0, s>>>(psi, np, bfac, axis, dcoef, vcoef, first ? 1 : 0,
+                                                   pos_d, mom_d);
+  return cudaGetLastError();
+}
+
+cudaError_t lpt_wrap(float* pos, int64_t n3, int ng, cudaStream_t s) {
+  lpt_wrap_kernel<<<grid_for(n3), 256, 0, s>>>(pos, n3, (float)ng, 1.f / ng);
+  return cudaGetLastError();
+}
+
+cudaError_t lpt_source(float* s, const float* a, const float* b, const float* c, int64_t n, int mode,
+                       cudaStream_t st) {
+  lpt_source_kernel<<<grid_for(n), 256, 0, st>>>(s, a, b, c, n, mode);
+  return cudaGetLastError();
+}
+
+}  // namespace fpm
