@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py -- PM steps/s and particle-updates/s of the FastPM force-and-update step on B200.
+
+Contract (see the task statement): `python bench.py --gpus N --steps K --warmup W` prints ONE JSON
+line on rank 0.  A "step" is one PM step of the whole hot path (paint -> r2c -> transfer function ->
+3x c2r -> readout -> kick -> drift) over all particles of the workload,
+executed by libfpm's fpm_pm_step (the loop body of fpm_nbody).  The workload is BASELINE.json's
+C4: 512^3 particles on a 512^3 mesh, 2LPT ICs at a = 0.1 (made by fpm_lpt_init from a seeded
+Eisenstein-Hu Gaussian field), stepped along C4's 40-step schedule so the particle distribution
+is the real, progressively clustered one.  Multi-GPU: replicas only -- each
+rank runs an independent simulation (seed + rank), no collective on the data path.
+
+`--impl reference` times the float64 CPU oracle (oracle/, test infrastructure) on the host cores
+on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import fpm_inputs as fi  # noqa: E402
+
+METRIC = "PM steps/sec at 512^3 (particle-updates/sec = value x 512^3)"
+FALLBACK_HBM_GBS = 6650.0
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes(n_p, ng):
+    """Algorithmic HBM bytes per launch of each kernel."""
+    n_g = ng ** 3
+    n_k = ng * ng * (ng // 2 + 1)
+    return {
+        "paint": 12 * n_p + 4 * n_g,
+        "fft_z_r2c": 4 * n_g + 8 * n_k,
+        "fft_cols_y": 16 * n_k,
+        "fft_cols_x": 16 * n_k,
+        "fft_z_c2r": 8 * n_k + 4 * n_g,
+        "apply_force_kernel": 32 * n_k,
+        "readout_kick_drift": 48 * n_p + 12 * n_g,
+        "readout": 24 * n_p + 12 * n_g,
+        "kick": 36 * n_p,
+        "drift": 36 * n_p,
+    }
+
+
+def step_bytes_unfused(n_p, ng):
+    """SURVEY.md 8(d) unfused model: 96 n_p + 112 n_g bytes per PM step."""
+    return 96 * n_p + 112 * ng ** 3
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap,power.draw")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                smax.append(float(r[1]))
+                power.append(float(r[6]))
+            except ValueError:
+                continue
+            for name, val in zip(names, r[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm),
+                "power_w_max": max(power) if power else None}
+
+
+def oracle_sample(cfg, n_side, n_steps):
+    """Times the float64 oracle on n_steps PM steps of an n_side^3 slice of the workload."""
+    import oracle
+    box = cfg.box * n_side / cfg.np_side          # same particle spacing as the workload
+    delta = fi.linear_field(n_side, box, cfg.seed).astype(np.float64)
+    om = fi.COSMO["omega_m"]
+    pos, mom = oracle.lpt_init(delta, n_side, om, cfg.a0, 1)
+    stages = cfg.stages()
+    times = []
+    for j in range(n_steps):
+        ai, af = stages[j], stages[j + 1]
+        ah = (ai * af) ** 0.5
+        t0 = time.perf_counter()
+        f = oracle.force(pos, n_side, scale=1.5 * om, mass=1.0)
+        mom = oracle.kick(mom, f, oracle.kick_factor(om, ai, ai, ah))
+        pos = oracle.drift(pos, mom, oracle.drift_factor(om, ai, ah, af), n_side)
+        times.append(time.perf_counter() - t0)
+    return times, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, same metric and unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = fi.CONFIGS[args.config]
+    n_side = min(cfg.np_side, 256 if args.ref_side is None else args.ref_side)
+    total = args.steps + args.warmup
+    times, cores = oracle_sample(cfg, n_side, total)
+    timed = times[args.warmup:]
+    upd_per_s = n_side ** 3 * len(timed) / sum(timed)
+    value = upd_per_s / cfg.n_particles
+    sample = (f"{len(timed)} PM steps (+{args.warmup} warm-up) of a {n_side}^3-particle / {n_side}^3-mesh slice "
+              f"of {cfg.name} (same particle spacing), float64 oracle; steps/s scaled by particle count "
+              f"{n_side}^3/{cfg.np_side}^3")
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "steps/s",
+        "particle_updates_per_sec": upd_per_s, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: {cfg.np_side}^3 particles on a {cfg.ng}^3 float32 mesh, box {cfg.box:g} Mpc/h, "
+            f"{cfg.lpt_order}LPT ICs at a={cfg.a0}, {cfg.n_steps}-step FastPM schedule linear in a to a={cfg.a1}")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C4", choices=sorted(fi.CONFIGS))
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-side", type=int, default=None)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2010_11847_b200 as fpm   # raises if libfpm.so is missing: no fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    cfg = fi.CONFIGS[args.config]
+    n_p, ng = cfg.n_particles, cfg.ng
+    ctx = fpm.FPM(ng, cfg.np_side, omega_m=fi.COSMO["omega_m"], box=cfg.box, device=device)
+
+    # ---- inputs: seeded Gaussian field -> 2LPT particles, all resident in HBM -----------------
+    delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, cfg.seed + rank)).to(device)
+    pos, mom = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
+    del delta
+    factors = ctx.step_factors(cfg.stages())
+
+    def fac(i):  # beyond the schedule keep stepping with the last full step's factors
+        return factors[i] if i < len(factors) - 1 else factors[len(factors) - 2]
+
+    step_no = 0
+    for _ in range(args.warmup):
+        ctx.pm_step(pos, mom, *fac(step_no))
+        step_no += 1
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ctx.profile_reset()
+    ctx.profile_enable(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    first_timed = step_no
+    for _ in range(args.steps):
+        ctx.pm_step(pos, mom, *fac(step_no))
+        step_no += 1
+    ev1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = ctx.launch_count()
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms_total], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / args.steps
+    value = world * 1e3 / ms_per_step          # whole-job steps/s (replicas)
+
+    # ---- end to end through the C-ABI with HOST buffers -----------------------------------------
+    e2e = None
+    if args.e2e_steps > 0:
+        h_pos = torch.empty((3, n_p), dtype=torch.float32, pin_memory=True)
+        h_mom = torch.empty((3, n_p), dtype=torch.float32, pin_memory=True)
+        h_pos.copy_(pos)
+        h_mom.copy_(mom)
+        torch.cuda.synchronize()
+        ctx.pm_step_host(h_pos, h_mom, pos, mom, *fac(step_no))   # warm-up
+        step_no += 1
+        if world > 1:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.e2e_steps):
+            ctx.pm_step_host(h_pos, h_mom, pos, mom, *fac(step_no))
+            step_no += 1
+        e1.record()
+        torch.cuda.synchronize()
+        e2e_ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        e2e = {"value": world * 1e3 * args.e2e_steps / e2e_ms, "unit": "steps/s",
+               "h2d_bytes_per_step": 24 * n_p, "d2h_bytes_per_step": 24 * n_p,
+               "steps": args.e2e_steps,
+               "call": "fpm_pm_step_host (pinned host pos+mom -> device, step, -> host)"}
+        del h_pos, h_mom
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- per-kernel roofline from the live CUDA-event profile ------------------------------------
+    peak, peak_src = measured_peaks()
+    abytes = algorithmic_bytes(n_p, ng)
+    kernels = {}
+    for name, (ms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        per = ms / cnt
+        k = {"launches_per_step": cnt / args.steps, "ms_per_launch": per, "ms_per_step": ms / args.steps}
+        if name in abytes:
+            k["algorithmic_bytes"] = abytes[name]
+            k["gbs"] = abytes[name] / per / 1e6
+            k["frac"] = k["gbs"] / peak
+        kernels[name] = k
+    dominant = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(args.config, {}).get(dominant)
+    dk = kernels[dominant]
+    roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk.get("gbs"), "peak": peak,
+                "unit": "GB/s", "frac": dk.get("frac"), "traffic": traffic, "peak_source": peak_src,
+                "share_of_step": dk["ms_per_step"] / ms_per_step}
+    step_gbs = step_bytes_unfused(n_p, ng) / ms_per_step / 1e6
+    step_roofline = {"algorithmic_bytes_per_step": step_bytes_unfused(n_p, ng), "achieved": step_gbs,
+                     "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
+                     "model": "96 n_p + 112 n_g (SURVEY.md 8(d), unfused)"}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        side = min(cfg.np_side, 256)
+        times, cores = oracle_sample(cfg, side, 3)
+        upd = side ** 3 * 2 / sum(times[1:])
+        cpu_baseline = {"value": upd / n_p, "unit": "steps/s", "cores": cores, "kind": "oracle",
+                        "particle_updates_per_sec": upd,
+                        "sample": f"2 PM steps (+1 warm-up) of a {side}^3-particle / {side}^3-mesh slice of "
+                                  f"{cfg.name}, float64 oracle, steps/s scaled by {side}^3/{cfg.np_side}^3"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": "steps/s",
+        "particle_updates_per_sec": value * n_p,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "timed_schedule_steps": [first_timed, first_timed + args.steps - 1],
+                   "l2_policy": "inputs larger than L2 (3.2 GB particle state, 0.5 GB meshes vs 126 MB L2)",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "kernel_mode": "paper Eq. 4+5", "force_path": "unfused"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

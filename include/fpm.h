@@ -151,6 +151,17 @@ int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, flo
 int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int n_steps,
               float* traj);
 
+/* One PM step = one force evaluation + kick + drift (the loop body of
+ * fpm_nbody): force at pos (paint, r2c, transfer function, 3 c2r, readout), mom += force *
+ * kick_fac, pos = wrap(pos + mom * drift_fac).  kick_fac / drift_fac: HOST doubles from
+ * fpm_kick_factor / fpm_drift_factor.  Needs the workspace. */
+int fpm_pm_step(fpm_ctx* ctx, float* pos, float* mom, int64_t n, double kick_fac,
+                double drift_fac);
+/* The same step with HOST state: h_pos/h_mom [3][n] are copied to d_pos/d_mom (DEVICE,
+ * caller-owned), stepped, copied back; synchronises before returning. */
+int fpm_pm_step_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom,
+                     int64_t n, double kick_fac, double drift_fac);
+
 /* The same run with HOST buffers: h_pos/h_mom [3][n] (pinned or pageable) are copied to the
  * device buffers d_pos/d_mom (DEVICE, caller-owned), evolved, copied back; synchronises. */
 int fpm_nbody_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom,
@@ -166,6 +177,17 @@ int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t
  * grad_out); grad_pos [3][n] = grad_out_p sum_c mesh[c] dW/dx_d (overwritten) or NULL. */
 int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n,
                         const float* grad_out, float* grad_mesh, float* grad_pos);
+
+/* ---- measurement hooks -------------------------------------------------------------------- */
+/* Per-kernel CUDA-event timing on the context's stream (off by default).  fpm_profile_read
+ * synchronises the recorded events; kernel_id runs over 0 .. until FPM_EINVAL is returned.
+ * name: HOST out (static string); total_ms / count: HOST out, accumulated since the last reset. */
+int fpm_profile_enable(fpm_ctx* ctx, int on);
+int fpm_profile_reset(fpm_ctx* ctx);
+int fpm_profile_read(fpm_ctx* ctx, int kernel_id, const char** name, double* total_ms,
+                     int64_t* count);
+/* Kernels of this library launched on this context since the last fpm_profile_reset. */
+int64_t fpm_launch_count(const fpm_ctx* ctx);
 
 #ifdef __cplusplus
 }

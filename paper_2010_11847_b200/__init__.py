@@ -58,6 +58,13 @@ def _load():
         "fpm_lpt_init": (i32, [vp, vp, dbl, i32, vp, vp]),
         "fpm_nbody": (i32, [vp, vp, vp, ctypes.POINTER(dbl), i32, vp]),
         "fpm_nbody_host": (i32, [vp, vp, vp, vp, vp, ctypes.POINTER(dbl), i32]),
+        "fpm_pm_step": (i32, [vp, vp, vp, i64, dbl, dbl]),
+        "fpm_pm_step_host": (i32, [vp, vp, vp, vp, vp, i64, dbl, dbl]),
+        "fpm_profile_enable": (i32, [vp, i32]),
+        "fpm_profile_reset": (i32, [vp]),
+        "fpm_profile_read": (i32, [vp, i32, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(dbl),
+                                   ctypes.POINTER(i64)]),
+        "fpm_launch_count": (i64, [vp]),
         "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
         "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
     }
@@ -214,6 +221,58 @@ class FPM:
         st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
         self._check(_lib.fpm_nbody(self._h, _dev(pos), _dev(mom), st, len(stages) - 1, _dev(traj)))
         return pos, mom
+
+    def pm_step(self, pos, mom, kick_fac, drift_fac):
+        """One PM step: force at pos, mom += f * kick_fac, pos = wrap(pos + mom * drift_fac)."""
+        self._check(_lib.fpm_pm_step(self._h, _dev(pos), _dev(mom), pos.shape[1], kick_fac, drift_fac))
+        return pos, mom
+
+    def pm_step_host(self, h_pos, h_mom, d_pos, d_mom, kick_fac, drift_fac):
+        """The same step on HOST float32 tensors: H2D, step, D2H, synchronise."""
+        for t in (h_pos, h_mom):
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+                raise FpmError("pm_step_host expects contiguous CPU float32 tensors")
+        self._check(_lib.fpm_pm_step_host(self._h, ctypes.c_void_p(h_pos.data_ptr()),
+                                          ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos), _dev(d_mom),
+                                          h_pos.shape[1], kick_fac, drift_fac))
+        return h_pos, h_mom
+
+    def step_factors(self, stages):
+        """(kick_fac, drift_fac) of the n+1 PM steps fpm_nbody performs for stages a_0..a_n."""
+        out, pending = [], 0.0
+        n = len(stages) - 1
+        for j in range(n + 1):
+            kf, dr = pending, 0.0
+            if j < n:
+                ai, af = float(stages[j]), float(stages[j + 1])
+                ah = (ai * af) ** 0.5
+                kf += self.kick_factor(ai, ai, ah)
+                dr = self.drift_factor(ai, ah, af)
+                pending = self.kick_factor(ah, af, af)
+            out.append((kf, dr))
+        return out
+
+    # ---- measurement hooks ----------------------------------------------------------------
+    def profile_enable(self, on=True):
+        self._check(_lib.fpm_profile_enable(self._h, int(bool(on))))
+
+    def profile_reset(self):
+        self._check(_lib.fpm_profile_reset(self._h))
+
+    def profile_read(self):
+        """{kernel name: (total ms, launches timed)} since the last reset (synchronises)."""
+        out, kid = {}, 0
+        while True:
+            name, ms, cnt = ctypes.c_char_p(), ctypes.c_double(), ctypes.c_int64()
+            rc = _lib.fpm_profile_read(self._h, kid, ctypes.byref(name), ctypes.byref(ms), ctypes.byref(cnt))
+            if rc != OK:
+                break
+            out[name.value.decode()] = (ms.value, cnt.value)
+            kid += 1
+        return out
+
+    def launch_count(self):
+        return int(_lib.fpm_launch_count(self._h))
 
     def nbody_host(self, h_pos, h_mom, d_pos, d_mom, stages):
         """Whole run on HOST float32 tensors (pinned for full PCIe speed); synchronises."""

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfpm.so")
-SOURCES = ["api.cu", "fft.cu", "mesh_ops.cu", "particles.cu", "green.cu", "cosmology.cpp"]
+SOURCES = ["api.cu", "fft.cu", "mesh_ops.cu", "particles.cu", "green.cu", "cosmology.cpp", "profiler.cpp"]
 HEADERS = ["fft.cuh", "fft_kernels.cuh", "fpm_internal.h", os.path.join("..", "..", "include", "fpm.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]

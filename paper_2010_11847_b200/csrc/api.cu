@@ -84,11 +84,26 @@ inline float particle_mass(const fpm_ctx* ctx) {
 int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n) {
   const int ng = ctx->cfg.ng;
   cudaStream_t s = ctx->stream;
-  FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, s));
-  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s));
-  FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, w.dk, (float)(1.5 * ctx->cfg.omega_m), w.fk[0], w.fk[1],
-                                   w.fk[2], s));
-  for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.fk[d], w.F[d], s));
+  Profiler* pr = &ctx->prof;
+  { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, s)); }
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
+  {
+    ProfScope sc(pr, K_GREEN);
+    FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, w.dk, (float)(1.5 * ctx->cfg.omega_m), w.fk[0],
+                                     w.fk[1], w.fk[2], s));
+  }
+  for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.fk[d], w.F[d], s, pr));
+  return FPM_OK;
+}
+
+// One PM step: force at the current positions, p += f K, x = wrap(x + p D).
+int pm_step(fpm_ctx* ctx, const Workspace& w, float* pos, float* mom, int64_t n, double kfac,
+            double dfac) {
+  const int rc = force_meshes(ctx, w, pos, n);
+  if (rc != FPM_OK) return rc;
+  ProfScope sc(&ctx->prof, K_READOUT_KICK_DRIFT);
+  FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
+                                   (float)dfac, ctx->stream));
   return FPM_OK;
 }
 
@@ -111,6 +126,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
   if (!ctx) return FPM_ENOMEM;
   ctx->cfg = *cfg;
   ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+  ctx->prof.stream = ctx->stream;
   cudaError_t e = fft_tables_create(cfg->ng, &ctx->fft_g);
   if (e == cudaSuccess) e = fft_tables_create(cfg->np, &ctx->fft_p);
   if (e == cudaSuccess) e = kernel_tables_create(cfg->ng, cfg->kernel_mode, &ctx->kt_g);
@@ -125,6 +141,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
 
 int fpm_destroy(fpm_ctx* ctx) {
   if (!ctx) return FPM_EINVAL;
+  ctx->prof.destroy();
   fft_tables_destroy(&ctx->fft_g);
   fft_tables_destroy(&ctx->fft_p);
   kernel_tables_destroy(&ctx->kt_g);
@@ -167,6 +184,7 @@ int fpm_kick_factor(const fpm_ctx* ctx, double ai, double ac, double af, double*
 int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, float* mesh) {
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && mesh && (pos || n == 0), "fpm_paint: bad arguments");
+  ProfScope sc(&ctx->prof, K_PAINT);
   FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, ctx->stream));
   return FPM_OK;
 }
@@ -176,7 +194,7 @@ int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx) {
   FPM_REQUIRE(ctx, real && cplx, "fpm_fft_r2c: null pointer");
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
               "fpm_fft_r2c: pointers must be 8-byte aligned");
-  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, real, reinterpret_cast<float2*>(cplx), ctx->stream));
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, real, reinterpret_cast<float2*>(cplx), ctx->stream, &ctx->prof));
   return FPM_OK;
 }
 
@@ -185,7 +203,7 @@ int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real) {
   FPM_REQUIRE(ctx, real && cplx, "fpm_fft_c2r: null pointer");
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
               "fpm_fft_c2r: pointers must be 8-byte aligned");
-  FPM_CUDA(ctx, fft_c2r(ctx->fft_g, reinterpret_cast<float2*>(cplx), real, ctx->stream));
+  FPM_CUDA(ctx, fft_c2r(ctx->fft_g, reinterpret_cast<float2*>(cplx), real, ctx->stream, &ctx->prof));
   return FPM_OK;
 }
 
@@ -195,6 +213,7 @@ int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, floa
   FPM_REQUIRE(ctx, delta_k && fkx && fky && fkz, "fpm_apply_force_kernel: null pointer");
   FPM_REQUIRE(ctx, delta_k != fkx && delta_k != fky && delta_k != fkz,
               "fpm_apply_force_kernel: outputs must not alias the input");
+  ProfScope sc(&ctx->prof, K_GREEN);
   FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, reinterpret_cast<const float2*>(delta_k), scale,
                                    reinterpret_cast<float2*>(fkx), reinterpret_cast<float2*>(fky),
                                    reinterpret_cast<float2*>(fkz), ctx->stream));
@@ -204,6 +223,7 @@ int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, floa
 int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, float* out) {
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && mesh && ((pos && out) || n == 0), "fpm_readout: bad arguments");
+  ProfScope sc(&ctx->prof, K_READOUT);
   FPM_CUDA(ctx, readout(mesh, pos, n, ctx->cfg.ng, out, ctx->stream));
   return FPM_OK;
 }
@@ -215,6 +235,7 @@ int fpm_force(fpm_ctx* ctx, const float* pos, int64_t n, float* force) {
   const Workspace w = carve(ctx);
   const int rc = force_meshes(ctx, w, pos, n);
   if (rc != FPM_OK) return rc;
+  ProfScope sc(&ctx->prof, K_READOUT);
   FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ctx->cfg.ng, force, ctx->stream));
   return FPM_OK;
 }
@@ -230,6 +251,7 @@ int fpm_kick(fpm_ctx* ctx, float* mom, const float* force, int64_t n, double ai,
   FPM_REQUIRE(ctx, n >= 0 && ((mom && force) || n == 0), "fpm_kick: bad arguments");
   FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_kick: scale factors must be positive");
   const double k = kick_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  ProfScope sc(&ctx->prof, K_KICK);
   FPM_CUDA(ctx, kick(mom, force, 3 * n, (float)k, ctx->stream));
   return FPM_OK;
 }
@@ -240,6 +262,7 @@ int fpm_drift(fpm_ctx* ctx, float* pos, const float* mom, int64_t n, double ai, 
   FPM_REQUIRE(ctx, n >= 0 && ((pos && mom) || n == 0), "fpm_drift: bad arguments");
   FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_drift: scale factors must be positive");
   const double d = drift_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  ProfScope sc(&ctx->prof, K_DRIFT);
   FPM_CUDA(ctx, drift(pos, mom, 3 * n, (float)d, ctx->cfg.ng, ctx->stream));
   return FPM_OK;
 }
@@ -260,40 +283,40 @@ int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, flo
   float2 *dk = w.dk, *tk = w.fk[0], *sk = w.fk[1];
   float *ra = w.F[0], *rb = w.F[1], *rc = w.F[2], *src = w.rho;
 
-  FPM_CUDA(ctx, fft_r2c(ctx->fft_p, delta_lin, dk, s));
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_p, delta_lin, dk, s, &ctx->prof));
   // psi1_d = c2r(i k_d delta / k^2);  x = q + D1 psi1,  p = a^2 E f1 D1 psi1   (1LPT / Zel'dovich)
   for (int d = 0; d < 3; ++d) {
-    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, d, -1, -1.f, s));
-    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
-    FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D1, (float)(pre * g.f1 * g.D1), true,
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, d, -1, -1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s, &ctx->prof));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D1, (float)(pre * g.f1 * g.D1), true,
                                pos + d * n3, mom + d * n3, s));
   }
   if (order == 2) {
     // S = sum_{i<j} (phi,ii phi,jj - phi,ij^2), phi,ij = c2r(k_i k_j delta / k^2)
-    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 0, 0, 1.f, s));
-    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
-    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 1, 1, 1.f, s));
-    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rb, s));
-    FPM_CUDA(ctx, lpt_source(src, ra, rb, nullptr, n3, 0, s));
-    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 2, 2, 1.f, s));
-    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rc, s));
-    FPM_CUDA(ctx, lpt_source(src, ra, rb, rc, n3, 1, s));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 0, 0, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s, &ctx->prof));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 1, 1, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rb, s, &ctx->prof));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_source(src, ra, rb, nullptr, n3, 0, s));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, 2, 2, 1.f, s));
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, rc, s, &ctx->prof));
+    ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_source(src, ra, rb, rc, n3, 1, s));
     const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
     for (auto& pr : pairs) {
-      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, pr[0], pr[1], 1.f, s));
-      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
-      FPM_CUDA(ctx, lpt_source(src, ra, nullptr, nullptr, n3, 2, s));
+      ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, pr[0], pr[1], 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s, &ctx->prof));
+      ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_source(src, ra, nullptr, nullptr, n3, 2, s));
     }
-    FPM_CUDA(ctx, fft_r2c(ctx->fft_p, src, sk, s));
+    FPM_CUDA(ctx, fft_r2c(ctx->fft_p, src, sk, s, &ctx->prof));
     // psi2_d = c2r(-i k_d S / k^2);  x += D2 psi2,  p += a^2 E f2 D2 psi2
     for (int d = 0; d < 3; ++d) {
-      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, sk, tk, d, -1, 1.f, s));
-      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s));
-      FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D2, (float)(pre * g.f2 * g.D2), false,
+      ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, sk, tk, d, -1, 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, ra, s, &ctx->prof));
+      ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_displace(ra, np, bfac, d, (float)g.D2, (float)(pre * g.f2 * g.D2), false,
                                  pos + d * n3, mom + d * n3, s));
     }
   }
-  FPM_CUDA(ctx, lpt_wrap(pos, 3 * n3, ng, s));
+  ctx->prof.launches += 1; FPM_CUDA(ctx, lpt_wrap(pos, 3 * n3, ng, s));
   return FPM_OK;
 }
 
@@ -306,30 +329,26 @@ int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int 
   FPM_NEED_WS(ctx);
   const Workspace w = carve(ctx);
   cudaStream_t s = ctx->stream;
-  const int ng = ctx->cfg.ng, np = ctx->cfg.np;
+  const int np = ctx->cfg.np;
   const int64_t n = (int64_t)np * np * np;
   const double om = ctx->cfg.omega_m;
   const int fm = ctx->cfg.factor_mode;
 
-  int rc = force_meshes(ctx, w, pos, n);
-  if (rc != FPM_OK) return rc;
-  if (traj) FPM_CUDA(ctx, cudaMemcpyAsync(traj, pos, sizeof(float) * 3 * n, cudaMemcpyDeviceToDevice, s));
   double pending_kick = 0.0;   // second half kick of the previous step, same force mesh
-  for (int j = 0; j < n_steps; ++j) {
-    const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
-    const double k1 = kick_factor(om, ai, ai, ah, fm);
-    const double dr = drift_factor(om, ai, ah, af, fm);
-    FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ng,
-                                     (float)(pending_kick + k1), (float)dr, s));
-    rc = force_meshes(ctx, w, pos, n);
-    if (rc != FPM_OK) return rc;
+  for (int j = 0; j <= n_steps; ++j) {
     if (traj)
-      FPM_CUDA(ctx, cudaMemcpyAsync(traj + (int64_t)(j + 1) * 3 * n, pos, sizeof(float) * 3 * n,
+      FPM_CUDA(ctx, cudaMemcpyAsync(traj + (int64_t)j * 3 * n, pos, sizeof(float) * 3 * n,
                                     cudaMemcpyDeviceToDevice, s));
-    pending_kick = kick_factor(om, ah, af, af, fm);
+    double kf = pending_kick, dr = 0.0;
+    if (j < n_steps) {
+      const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
+      kf += kick_factor(om, ai, ai, ah, fm);
+      dr = drift_factor(om, ai, ah, af, fm);
+      pending_kick = kick_factor(om, ah, af, af, fm);
+    }
+    const int rc = pm_step(ctx, w, pos, mom, n, kf, dr);
+    if (rc != FPM_OK) return rc;
   }
-  if (n_steps > 0)
-    FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ng, (float)pending_kick, 0.f, s));
   return FPM_OK;
 }
 
@@ -350,10 +369,59 @@ int fpm_nbody_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float
   return FPM_OK;
 }
 
+int fpm_pm_step(fpm_ctx* ctx, float* pos, float* mom, int64_t n, double kick_fac, double drift_fac) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((pos && mom) || n == 0), "fpm_pm_step: bad arguments");
+  FPM_REQUIRE(ctx, std::isfinite(kick_fac) && std::isfinite(drift_fac), "fpm_pm_step: non-finite factor");
+  FPM_NEED_WS(ctx);
+  return pm_step(ctx, carve(ctx), pos, mom, n, kick_fac, drift_fac);
+}
+
+int fpm_pm_step_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom, int64_t n,
+                     double kick_fac, double drift_fac) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && h_pos && h_mom && d_pos && d_mom, "fpm_pm_step_host: bad arguments");
+  const size_t bytes = sizeof(float) * 3 * (size_t)n;
+  cudaStream_t s = ctx->stream;
+  FPM_CUDA(ctx, cudaMemcpyAsync(d_pos, h_pos, bytes, cudaMemcpyHostToDevice, s));
+  FPM_CUDA(ctx, cudaMemcpyAsync(d_mom, h_mom, bytes, cudaMemcpyHostToDevice, s));
+  const int rc = fpm_pm_step(ctx, d_pos, d_mom, n, kick_fac, drift_fac);
+  if (rc != FPM_OK) return rc;
+  FPM_CUDA(ctx, cudaMemcpyAsync(h_pos, d_pos, bytes, cudaMemcpyDeviceToHost, s));
+  FPM_CUDA(ctx, cudaMemcpyAsync(h_mom, d_mom, bytes, cudaMemcpyDeviceToHost, s));
+  FPM_CUDA(ctx, cudaStreamSynchronize(s));
+  return FPM_OK;
+}
+
+int fpm_profile_enable(fpm_ctx* ctx, int on) {
+  if (!ctx) return FPM_EINVAL;
+  ctx->prof.flush();
+  ctx->prof.enabled = on != 0;
+  return FPM_OK;
+}
+
+int fpm_profile_reset(fpm_ctx* ctx) {
+  if (!ctx) return FPM_EINVAL;
+  ctx->prof.reset();
+  return FPM_OK;
+}
+
+int fpm_profile_read(fpm_ctx* ctx, int kernel_id, const char** name, double* total_ms, int64_t* count) {
+  if (!ctx || kernel_id < 0 || kernel_id >= K_COUNT) return FPM_EINVAL;
+  ctx->prof.flush();
+  if (name) *name = kernel_name(kernel_id);
+  if (total_ms) *total_ms = ctx->prof.ms[kernel_id];
+  if (count) *count = ctx->prof.count[kernel_id];
+  return FPM_OK;
+}
+
+int64_t fpm_launch_count(const fpm_ctx* ctx) { return ctx ? ctx->prof.launches : -1; }
+
 int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n,
                       const float* grad_mesh, float* grad_pos, float* grad_mass) {
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_pos) || n == 0), "fpm_paint_adjoint: bad arguments");
+  ProfScope sc(&ctx->prof, K_READOUT_GRAD);
   FPM_CUDA(ctx, readout_grad(grad_mesh, pos, mass, particle_mass(ctx), n, ctx->cfg.ng, grad_pos,
                              grad_mass, ctx->stream));
   return FPM_OK;
@@ -364,9 +432,11 @@ int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_out) || n == 0), "fpm_readout_adjoint: bad arguments");
   FPM_REQUIRE(ctx, !grad_pos || mesh, "fpm_readout_adjoint: grad_pos needs the forward mesh");
-  FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, ctx->stream));
-  if (grad_pos)
+  { ProfScope sc(&ctx->prof, K_PAINT); FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, ctx->stream)); }
+  if (grad_pos) {
+    ProfScope sc(&ctx->prof, K_READOUT_GRAD);
     FPM_CUDA(ctx, readout_grad(mesh, pos, grad_out, 0.f, n, ctx->cfg.ng, grad_pos, nullptr, ctx->stream));
+  }
   return FPM_OK;
 }
 

@@ -64,10 +64,12 @@ cudaError_t launch_cols(const float2* in, float2* out, int batches, int64_t batc
 }
 
 template <int N>
-cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaStream_t s) {
+cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaStream_t s,
+                     Profiler* prof) {
   constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
   const int64_t nrows = (int64_t)N * N;
   {
+    ProfScope sc(prof, K_FFT_Z_R2C);
     constexpr int threads = G * Plan<M>::P;
     const size_t smem = sizeof(float2) * G * row_pitch(M);
     auto kern = fft_z_r2c_kernel<N>;
@@ -78,20 +80,33 @@ cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaSt
     if (e != cudaSuccess) return e;
   }
   // y: one batch per x slab, columns kz, lines y (stride nzh)
-  cudaError_t e = launch_cols<N, false>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  cudaError_t e;
+  {
+    ProfScope sc(prof, K_FFT_Y);
+    e = launch_cols<N, false>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  }
   if (e != cudaSuccess) return e;
   // x: columns (y, kz) flattened, lines x (stride N nzh)
+  ProfScope sc(prof, K_FFT_X);
   return launch_cols<N, false>(cplx, cplx, 1, 0, N * nzh, (int64_t)N * nzh, t.stage_n, s);
 }
 
 template <int N>
-cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t s) {
+cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
   constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
   const int64_t nrows = (int64_t)N * N;
-  cudaError_t e = launch_cols<N, true>(cplx, cplx, 1, 0, N * nzh, (int64_t)N * nzh, t.stage_n, s);
+  cudaError_t e;
+  {
+    ProfScope sc(prof, K_FFT_X);
+    e = launch_cols<N, true>(cplx, cplx, 1, 0, N * nzh, (int64_t)N * nzh, t.stage_n, s);
+  }
   if (e != cudaSuccess) return e;
-  e = launch_cols<N, true>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  {
+    ProfScope sc(prof, K_FFT_Y);
+    e = launch_cols<N, true>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+  }
   if (e != cudaSuccess) return e;
+  ProfScope sc(prof, K_FFT_Z_C2R);
   constexpr int threads = G * Plan<M>::P;
   const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
   auto kern = fft_z_c2r_kernel<N>;
@@ -147,11 +162,12 @@ void fft_tables_destroy(FftTables* t) {
     default: return cudaErrorInvalidValue;               \
   }
 
-cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s) {
-  FPM_FFT_DISPATCH(r2c_impl, t, real, cplx, s)
+cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s,
+                    Profiler* prof) {
+  FPM_FFT_DISPATCH(r2c_impl, t, real, cplx, s, prof)
 }
-cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s) {
-  FPM_FFT_DISPATCH(c2r_impl, t, cplx, real, s)
+cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
+  FPM_FFT_DISPATCH(c2r_impl, t, cplx, real, s, prof)
 }
 
 }  // namespace fpm

@@ -4,10 +4,42 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/fpm.h"
 
 namespace fpm {
+
+// ---- per-kernel accounting: launch counter (always) + CUDA-event timing (when enabled) --------
+enum KernelId {
+  K_PAINT = 0, K_FFT_Z_R2C, K_FFT_Y, K_FFT_X, K_FFT_Z_C2R, K_GREEN, K_READOUT, K_READOUT_KICK_DRIFT,
+  K_KICK, K_DRIFT, K_READOUT_GRAD, K_LPT, K_COUNT
+};
+const char* kernel_name(int kid);
+
+struct Profiler {
+  bool enabled = false;
+  cudaStream_t stream = nullptr;
+  struct Rec { int kid; cudaEvent_t a, b; };
+  std::vector<cudaEvent_t> pool;
+  std::vector<Rec> open;
+  double ms[K_COUNT] = {0};
+  long long count[K_COUNT] = {0};
+  long long launches = 0;          // kernels of this library launched since the last reset
+  void begin(int kid);
+  void end();
+  void flush();                    // synchronises the recorded events and accumulates ms[]
+  void reset();
+  void destroy();
+};
+
+struct ProfScope {
+  Profiler* p;
+  ProfScope(Profiler* prof, int kid, int nlaunch = 1) : p(prof) {
+    if (p) { p->launches += nlaunch; p->begin(kid); }
+  }
+  ~ProfScope() { if (p) p->end(); }
+};
 
 // ---- FFT (fft.cu) ---------------------------------------------------------------------------
 struct FftTables {
@@ -36,8 +68,10 @@ void kernel_tables_destroy(KernelTables* t);
 // element-wise epilogue/prologue selectors for the fused x passes (fft.cu)
 enum XOp { XOP_NONE = 0, XOP_INVLAP = 1, XOP_GRAD = 2 };
 
-cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s);
-cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s);
+cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s,
+                    Profiler* prof = nullptr);
+cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s,
+                    Profiler* prof = nullptr);
 
 // ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
 cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
@@ -88,4 +122,5 @@ struct fpm_ctx {
   size_t ws_bytes = 0;
   bool sticky = false;
   std::string err;
+  fpm::Profiler prof;
 };
