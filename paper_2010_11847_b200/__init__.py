@@ -9,6 +9,8 @@ import os
 
 import torch
 
+from . import build as _build
+
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libfpm.so")
 
@@ -30,10 +32,11 @@ class _Config(ctypes.Structure):
 
 
 def _load():
-    if not os.path.exists(_LIB_PATH):
-        raise ImportError(
-            f"{_LIB_PATH} is missing: build it with `python -m paper_2010_11847_b200.build` "
-            "(nvcc, sm_100a). There is no CPU fallback.")
+    try:
+        _build.build()            # no-op when libfpm.so matches the sources (content hash)
+    except Exception as e:        # noqa: BLE001
+        raise ImportError(f"cannot build {_LIB_PATH} with nvcc for sm_100a ({e}); "
+                          "there is no CPU fallback") from e
     lib = ctypes.CDLL(_LIB_PATH)
     vp, i64, dbl, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
     sig = {

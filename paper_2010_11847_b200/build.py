@@ -1,4 +1,11 @@
-"""Builds libfpm.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+"""Builds libfpm.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+Staleness is decided by a content hash of the sources and flags kept beside the library
+(libfpm.so.stamp), not by mtimes, so a snapshot copied to another machine is not rebuilt.
+This module must stay importable without the built library (it is what builds it).
+"""
+import glob
+import hashlib
 import os
 import subprocess
 import sys
@@ -6,46 +13,68 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfpm.so")
-SOURCES = ["api.cu", "fft.cu", "mesh_ops.cu", "particles.cu", "green.cu", "cosmology.cpp", "profiler.cpp"]
-HEADERS = ["fft.cuh", "fft_kernels.cuh", "fpm_internal.h", os.path.join("..", "..", "include", "fpm.h")]
+STAMP = LIB + ".stamp"
+INCLUDE = os.path.join(HERE, "..", "include")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
 
 def _nvcc():
-    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
-        if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
+    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc"):
+        if cand and os.path.exists(cand):
             return cand
     return "nvcc"
 
 
+def sources():
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
+
+
+def _headers():
+    return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) +
+                  glob.glob(os.path.join(INCLUDE, "*.h")))
+
+
+def _digest():
+    h = hashlib.sha256()
+    h.update(" ".join(NVCC_FLAGS[:-1]).encode())
+    for path in sources() + _headers():
+        h.update(os.path.basename(path).encode())
+        with open(path, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
 def stale():
-    if not os.path.exists(LIB):
+    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != _digest()
 
 
 def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    objs = []
-    procs = []
+    digest = _digest()
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
-    for src in SOURCES:
-        obj = os.path.join(HERE, "build", src.rsplit(".", 1)[0] + ".o")
-        cmd = [_nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-x", "cu", "-c", os.path.join(CSRC, src), "-o", obj]
+    objs, procs = [], []
+    for src in sources():
+        obj = os.path.join(HERE, "build", os.path.basename(src).rsplit(".", 1)[0] + ".o")
+        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-x", "cu", "-c", src, "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
+    failed = []
     for src, p in procs:
         out, _ = p.communicate()
         if verbose or p.returncode != 0:
             sys.stderr.write(out)
         if p.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {src}")
+            failed.append(src)
+    if failed:
+        raise RuntimeError(f"nvcc failed on {failed}")
     subprocess.run([_nvcc(), "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"], check=True)
+    with open(STAMP, "w") as f:
+        f.write(digest + "\n")
     return LIB
 
 
