@@ -51,6 +51,8 @@ def algorithmic_bytes(n_p, ng):
         "fft_cols_x": 16 * n_k,
         "fft_z_c2r": 8 * n_k + 4 * n_g,
         "apply_force_kernel": 32 * n_k,
+        "fft_x_force": 24 * n_k,
+        "fft_y_inv3": 40 * n_k,
         "readout_kick_drift": 48 * n_p + 12 * n_g,
         "readout": 24 * n_p + 12 * n_g,
         "kick": 36 * n_p,
@@ -179,6 +181,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-side", type=int, default=None)
+    ap.add_argument("--force-path", default="fused", choices=["fused", "unfused"])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -200,7 +203,8 @@ def main():
 
     cfg = fi.CONFIGS[args.config]
     n_p, ng = cfg.n_particles, cfg.ng
-    ctx = fpm.FPM(ng, cfg.np_side, omega_m=fi.COSMO["omega_m"], box=cfg.box, device=device)
+    ctx = fpm.FPM(ng, cfg.np_side, omega_m=fi.COSMO["omega_m"], box=cfg.box, device=device,
+                  force_path=fpm.FORCE_FUSED if args.force_path == "fused" else fpm.FORCE_UNFUSED)
 
     # ---- inputs: seeded Gaussian field -> 2LPT particles, all resident in HBM -----------------
     delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, cfg.seed + rank)).to(device)
@@ -331,7 +335,7 @@ def main():
         "config": {"workload": workload_name(cfg), "timed_schedule_steps": [first_timed, first_timed + args.steps - 1],
                    "l2_policy": "inputs larger than L2 (3.2 GB particle state, 0.5 GB meshes vs 126 MB L2)",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "kernel_mode": "paper Eq. 4+5", "force_path": "unfused"},
+                   "kernel_mode": "paper Eq. 4+5", "force_path": args.force_path},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "cpu_baseline": cpu_baseline,

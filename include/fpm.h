@@ -59,6 +59,14 @@ enum {
   FPM_FORCE_FUSED = 1    /* Green's function fused into the FFT passes, readout+kick+drift fused */
 };
 
+/* How fpm_paint scatters (results agree within fp32 summation order). */
+enum {
+  FPM_PAINT_AUTO = 0,        /* brick window when the particles are a full np^3 lattice set, ng == np */
+  FPM_PAINT_DIRECT = 1,      /* one thread per particle, 8 global fp32 reductions */
+  FPM_PAINT_BRICK_FLOAT = 2, /* shared-memory window per lattice brick, fp32 accumulation */
+  FPM_PAINT_BRICK_FIXED = 3  /* shared-memory window per lattice brick, 32-bit fixed-point accumulation */
+};
+
 typedef struct {
   int32_t ng;          /* mesh cells per side */
   int32_t np;          /* particles per side (np^3 particles on a lattice of spacing ng/np) */
@@ -67,7 +75,7 @@ typedef struct {
   int32_t kernel_mode; /* FPM_KERNEL_* */
   int32_t factor_mode; /* FPM_FACTORS_* */
   int32_t force_path;  /* FPM_FORCE_* */
-  int32_t reserved;    /* must be 0 */
+  int32_t paint_mode;  /* FPM_PAINT_* */
 } fpm_config;
 
 typedef struct fpm_ctx fpm_ctx;
@@ -88,6 +96,9 @@ const char* fpm_last_error(const fpm_ctx* ctx);
 size_t fpm_workspace_bytes(const fpm_config* cfg);
 /* ws: DEVICE, 256-byte aligned, stays owned by the caller and must outlive its use. */
 int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes);
+
+/* Changes cfg.paint_mode after creation.  FPM_EINVAL on an unknown mode. */
+int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode);
 
 /* ---- background cosmology (host, float64; paper defers to Feng et al. 2016) -- */
 /* out: HOST double[7] = {D1, f1, D2, f2, E, Gf = a^3 E dD1/da, gf = dGf/da}, D1(1) = 1. */

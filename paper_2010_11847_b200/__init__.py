@@ -17,6 +17,7 @@ _LIB_PATH = os.path.join(_HERE, "libfpm.so")
 KERNEL_PAPER, KERNEL_NAIVE, KERNEL_MIXED = 0, 1, 2
 FACTORS_FASTPM, FACTORS_QUINN = 0, 1
 FORCE_UNFUSED, FORCE_FUSED = 0, 1
+PAINT_AUTO, PAINT_DIRECT, PAINT_BRICK_FLOAT, PAINT_BRICK_FIXED = 0, 1, 2, 3
 OK, EINVAL, ENOMEM, ECUDA, ENOTIMPL = 0, -1, -2, -3, -4
 
 
@@ -28,7 +29,7 @@ class _Config(ctypes.Structure):
     _fields_ = [("ng", ctypes.c_int32), ("np", ctypes.c_int32), ("omega_m", ctypes.c_double),
                 ("box", ctypes.c_double), ("kernel_mode", ctypes.c_int32),
                 ("factor_mode", ctypes.c_int32), ("force_path", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("paint_mode", ctypes.c_int32)]
 
 
 def _load():
@@ -46,6 +47,7 @@ def _load():
         "fpm_last_error": (ctypes.c_char_p, [vp]),
         "fpm_workspace_bytes": (ctypes.c_size_t, [ctypes.POINTER(_Config)]),
         "fpm_set_workspace": (i32, [vp, vp, ctypes.c_size_t]),
+        "fpm_set_paint_mode": (i32, [vp, i32]),
         "fpm_growth": (i32, [vp, dbl, ctypes.POINTER(dbl)]),
         "fpm_drift_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
         "fpm_kick_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
@@ -102,7 +104,7 @@ class FPM:
 
     def __init__(self, ng, np_side=None, omega_m=0.3075, box=0.0, kernel_mode=KERNEL_PAPER,
                  factor_mode=FACTORS_FASTPM, force_path=FORCE_UNFUSED, device="cuda:0",
-                 stream=None, workspace=True):
+                 stream=None, workspace=True, paint_mode=PAINT_AUTO):
         if not torch.cuda.is_available():
             raise FpmError("CUDA device required: libfpm has no CPU fallback")
         self.device = torch.device(device)
@@ -111,7 +113,7 @@ class FPM:
         self.nzh = self.ng // 2 + 1
         self.omega_m = float(omega_m)
         self._cfg = _Config(self.ng, self.np_side, self.omega_m, float(box), kernel_mode,
-                            factor_mode, force_path, 0)
+                            factor_mode, force_path, paint_mode)
         with torch.cuda.device(self.device):
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = ctypes.c_void_p()
@@ -144,6 +146,9 @@ class FPM:
 
     def _empty(self, *shape, dtype=torch.float32):
         return torch.empty(*shape, dtype=dtype, device=self.device)
+
+    def set_paint_mode(self, mode):
+        self._check(_lib.fpm_set_paint_mode(self._h, int(mode)))
 
     # ---- cosmology ----------------------------------------------------------------------
     def growth(self, a):

@@ -24,7 +24,7 @@ bool config_ok(const fpm_config* c) {
   if (c->kernel_mode < FPM_KERNEL_PAPER || c->kernel_mode > FPM_KERNEL_MIXED) return false;
   if (c->factor_mode < FPM_FACTORS_FASTPM || c->factor_mode > FPM_FACTORS_QUINN) return false;
   if (c->force_path < FPM_FORCE_UNFUSED || c->force_path > FPM_FORCE_FUSED) return false;
-  if (c->reserved != 0) return false;
+  if (c->paint_mode < FPM_PAINT_AUTO || c->paint_mode > FPM_PAINT_BRICK_FIXED) return false;
   return true;
 }
 
@@ -75,6 +75,14 @@ int cuda_fail(fpm_ctx* ctx, cudaError_t e, const char* where) {
   if (!(ctx)->ws || (ctx)->ws_bytes < fpm_workspace_bytes(&(ctx)->cfg)) \
     return fail((ctx), FPM_ENOMEM, "workspace missing or too small (fpm_set_workspace)");
 
+inline ParticleOrder order_of(const fpm_ctx* ctx, int64_t n) {
+  ParticleOrder o;
+  const int64_t np = ctx->cfg.np;
+  o.np = (n == np * np * np) ? (int)np : 0;
+  o.paint_mode = ctx->cfg.paint_mode;
+  return o;
+}
+
 inline float particle_mass(const fpm_ctx* ctx) {
   const float b = (float)(ctx->cfg.ng / ctx->cfg.np);
   return b * b * b;
@@ -85,7 +93,12 @@ int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n) 
   const int ng = ctx->cfg.ng;
   cudaStream_t s = ctx->stream;
   Profiler* pr = &ctx->prof;
-  { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, s)); }
+  { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s)); }
+  if (ctx->cfg.force_path == FPM_FORCE_FUSED) {
+    FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F,
+                                  (float)(1.5 * ctx->cfg.omega_m), s, pr));
+    return FPM_OK;
+  }
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
   {
     ProfScope sc(pr, K_GREEN);
@@ -103,7 +116,7 @@ int pm_step(fpm_ctx* ctx, const Workspace& w, float* pos, float* mom, int64_t n,
   if (rc != FPM_OK) return rc;
   ProfScope sc(&ctx->prof, K_READOUT_KICK_DRIFT);
   FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
-                                   (float)dfac, ctx->stream));
+                                   (float)dfac, order_of(ctx, n), ctx->stream));
   return FPM_OK;
 }
 
@@ -162,6 +175,13 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
   return FPM_OK;
 }
 
+int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, paint_mode >= FPM_PAINT_AUTO && paint_mode <= FPM_PAINT_BRICK_FIXED, "unknown paint mode");
+  ctx->cfg.paint_mode = paint_mode;
+  return FPM_OK;
+}
+
 int fpm_growth(const fpm_ctx* ctx, double a, double* out) {
   if (!ctx || !out || !(a > 0.0)) return FPM_EINVAL;
   const GrowthOut g = growth(ctx->cfg.omega_m, a);
@@ -185,7 +205,7 @@ int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, floa
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && mesh && (pos || n == 0), "fpm_paint: bad arguments");
   ProfScope sc(&ctx->prof, K_PAINT);
-  FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, ctx->stream));
+  FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, order_of(ctx, n), ctx->stream));
   return FPM_OK;
 }
 
@@ -224,7 +244,7 @@ int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, fl
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && mesh && ((pos && out) || n == 0), "fpm_readout: bad arguments");
   ProfScope sc(&ctx->prof, K_READOUT);
-  FPM_CUDA(ctx, readout(mesh, pos, n, ctx->cfg.ng, out, ctx->stream));
+  FPM_CUDA(ctx, readout(mesh, pos, n, ctx->cfg.ng, out, order_of(ctx, n), ctx->stream));
   return FPM_OK;
 }
 
@@ -236,7 +256,7 @@ int fpm_force(fpm_ctx* ctx, const float* pos, int64_t n, float* force) {
   const int rc = force_meshes(ctx, w, pos, n);
   if (rc != FPM_OK) return rc;
   ProfScope sc(&ctx->prof, K_READOUT);
-  FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ctx->cfg.ng, force, ctx->stream));
+  FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ctx->cfg.ng, force, order_of(ctx, n), ctx->stream));
   return FPM_OK;
 }
 
@@ -432,7 +452,7 @@ int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_out) || n == 0), "fpm_readout_adjoint: bad arguments");
   FPM_REQUIRE(ctx, !grad_pos || mesh, "fpm_readout_adjoint: grad_pos needs the forward mesh");
-  { ProfScope sc(&ctx->prof, K_PAINT); FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, ctx->stream)); }
+  { ProfScope sc(&ctx->prof, K_PAINT); FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, order_of(ctx, n), ctx->stream)); }
   if (grad_pos) {
     ProfScope sc(&ctx->prof, K_READOUT_GRAD);
     FPM_CUDA(ctx, readout_grad(mesh, pos, grad_out, 0.f, n, ctx->cfg.ng, grad_pos, nullptr, ctx->stream));

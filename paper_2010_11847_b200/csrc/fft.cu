@@ -92,9 +92,24 @@ cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaSt
 }
 
 template <int N>
-cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
-  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
+cudaError_t launch_z_c2r(const FftTables& t, const float2* cplx, float* real, const float* gz,
+                         cudaStream_t s, Profiler* prof) {
+  constexpr int M = N / 2, G = z_rows<N>();
   const int64_t nrows = (int64_t)N * N;
+  ProfScope sc(prof, K_FFT_Z_C2R);
+  constexpr int threads = G * Plan<M>::P;
+  const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
+  auto kern = fft_z_c2r_kernel<N>;
+  cudaError_t e = set_smem(kern, smem);
+  if (e != cudaSuccess) return e;
+  const float scale = (float)(1.0 / ((double)N * N * N));
+  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz);
+  return cudaGetLastError();
+}
+
+template <int N>
+cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
+  constexpr int nzh = N / 2 + 1;
   cudaError_t e;
   {
     ProfScope sc(prof, K_FFT_X);
@@ -106,15 +121,64 @@ cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t
     e = launch_cols<N, true>(cplx, cplx, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
   }
   if (e != cudaSuccess) return e;
-  ProfScope sc(prof, K_FFT_Z_C2R);
-  constexpr int threads = G * Plan<M>::P;
-  const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
-  auto kern = fft_z_c2r_kernel<N>;
-  e = set_smem(kern, smem);
+  return launch_z_c2r<N>(t, cplx, real, nullptr, s, prof);
+}
+
+// Fused force meshes: r2c z, y forward, x round trip with the transfer
+// function (2 variants), 3 inverse y passes in one launch, 3 c2r z passes (g(w_z) fused into the
+// third).  wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.
+template <int N>
+cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
+                             float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                             cudaStream_t s, Profiler* prof) {
+  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>(), T = col_tile<N>();
+  const int64_t nrows = (int64_t)N * N;
+  cudaError_t e;
+  {
+    ProfScope sc(prof, K_FFT_Z_R2C);
+    constexpr int threads = G * Plan<M>::P;
+    const size_t smem = sizeof(float2) * G * row_pitch(M);
+    auto kern = fft_z_r2c_kernel<N>;
+    e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(rho, dk, nrows, t.stage_m, t.full);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  {
+    ProfScope sc(prof, K_FFT_Y);
+    e = launch_cols<N, false>(dk, dk, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    if (e != cudaSuccess) return e;
+  }
+  constexpr int threads = T * Plan<N>::P;
+  const size_t smem = Plan<N>::NST > 1 ? sizeof(float2) * N * T : 0;
+  {
+    ProfScope sc(prof, K_FFT_X_FORCE);
+    auto kern = fft_x_force_kernel<N>;
+    e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    const int ncols = N * nzh;
+    kern<<<2 * ((ncols + T - 1) / T), threads, smem, s>>>(dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_n,
+                                                        kt.lap, kt.grad, scale);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  {
+    ProfScope sc(prof, K_FFT_Y_INV3);
+    auto kern = fft_y_inv3_kernel<N>;
+    e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(3 * ((nzh + T - 1) / T), N);
+    // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
+    kern<<<grid, threads, smem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * nzh, nzh, nzh, t.stage_n, kt.grad);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof);
   if (e != cudaSuccess) return e;
-  const float scale = (float)(1.0 / ((double)N * N * N));
-  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale);
-  return cudaGetLastError();
+  e = launch_z_c2r<N>(t, dk, F[1], nullptr, s, prof);
+  if (e != cudaSuccess) return e;
+  return launch_z_c2r<N>(t, wc, F[2], kt.grad, s, prof);
 }
 
 }  // namespace
@@ -168,6 +232,13 @@ cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStr
 }
 cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
   FPM_FFT_DISPATCH(c2r_impl, t, cplx, real, s, prof)
+}
+
+cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
+                            float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                            cudaStream_t s, Profiler* prof) {
+  if (kt.n != t.n) return cudaErrorInvalidValue;
+  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, scale, s, prof)
 }
 
 }  // namespace fpm

@@ -55,6 +55,88 @@ fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
   }
 }
 
+// Fused transfer function (Eq. 3-5) on the x axis: forward x transform of the
+// y-transformed density, times  i s / K^2  (variant 0: "A")  or  i s g(w_x) / K^2  (variant 1: "Bx"),
+// inverse x transform, all inside one block -- delta_k, and the three force spectra of the unfused
+// path, never reach HBM.  Since g(w_y) and g(w_z) are constant along x, F_y and F_z follow from A
+// by a multiplication in the y and z passes.  Block b: tile b >> 1, variant b & 1 (the two readers
+// of a tile run back to back, so the second read is an L2 hit).
+// columns = flattened (y, kz), lines = x with stride line_stride; no normalisation here.
+template <int N>
+__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
+                   float2* __restrict__ out_bx, int ncols, int nzh, int64_t line_stride,
+                   const float2* __restrict__ tw, const float* __restrict__ lap,
+                   const float* __restrict__ grad, float scale) {
+  extern __shared__ float2 smem[];
+  using PL = Plan<N>;
+  constexpr int T = col_tile<N>(), E = PL::E, P = PL::P;
+  const int c = threadIdx.x % T, p = threadIdx.x / T;
+  const int variant = blockIdx.x & 1;
+  const int64_t col = (int64_t)(blockIdx.x >> 1) * T + c;
+  const bool ok = col < ncols;
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    v[e] = ok ? in[col + (int64_t)(p + P * e) * line_stride] : make_float2(0.f, 0.f);
+  ColSmem<T> sm{smem, c};
+  fft_line<N>(v, p, sm, tw);
+  const int y = ok ? (int)(col / nzh) : 0, kz = ok ? (int)(col % nzh) : 0;
+  const float lyz = __ldg(lap + y) + __ldg(lap + kz);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    const float k2 = __ldg(lap + i) + lyz;
+    float f = (col == 0 && i == 0) ? 0.f : scale / k2;
+    if (variant) f *= __ldg(grad + i);
+    // i f v = (-im, re) f ; stored (im, re)-swapped for the inverse transform
+    v[e] = make_float2(v[e].x * f, -v[e].y * f);
+  }
+  if constexpr (PL::NST > 1) __syncthreads();
+  fft_line<N>(v, p, sm, tw);
+  if (ok) {
+    float2* out = variant ? out_bx : out_a;
+#pragma unroll
+    for (int e = 0; e < E; ++e) out[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
+  }
+}
+
+// The three inverse y passes of the fused force path in one launch.  Block b: tile b / 3 of x slab
+// blockIdx.y, variant b % 3:  0: Bx -> Fx (in place),  1: g(w_y) A -> Fy,  2: A -> Fz (g(w_z) is applied
+// by the z pass).  in0/out0 may alias; A is read by variants 1 and 2 and written by neither.
+template <int N>
+__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
+                  float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
+                  int ncols, int64_t line_stride, const float2* __restrict__ tw,
+                  const float* __restrict__ grad) {
+  extern __shared__ float2 smem[];
+  using PL = Plan<N>;
+  constexpr int T = col_tile<N>(), E = PL::E, P = PL::P;
+  const int c = threadIdx.x % T, p = threadIdx.x / T;
+  const int variant = blockIdx.x % 3;
+  const int64_t col = (int64_t)(blockIdx.x / 3) * T + c;
+  const bool ok = col < ncols;
+  const int64_t off = (int64_t)blockIdx.y * batch_stride + col;
+  const float2* in = variant == 0 ? in_bx : in_a;
+  float2* out = variant == 0 ? out_x : (variant == 1 ? out_y : out_z);
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    float2 x = make_float2(0.f, 0.f);
+    if (ok) x = in[off + (int64_t)i * line_stride];
+    if (variant == 1) { const float g = __ldg(grad + i); x.x *= g; x.y *= g; }
+    v[e] = cswap(x);
+  }
+  ColSmem<T> sm{smem, c};
+  fft_line<N>(v, p, sm, tw);
+  if (ok) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) out[off + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
+  }
+}
+
 // real rows of N floats -> rows of N/2+1 complex.  twn[k] = exp(-2 pi i k / N), k < N/2.
 template <int N>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
@@ -101,7 +183,8 @@ fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t
 template <int N>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
 fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t nrows,
-                 const float2* __restrict__ tw, const float2* __restrict__ twn, float scale) {
+                 const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
+                 const float* __restrict__ gz) {
   extern __shared__ float2 smem[];
   constexpr int M = N / 2;
   using PL = Plan<M>;
@@ -116,7 +199,11 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
     const int k = p + P * e;
     float2 z = make_float2(0.f, 0.f);
     if (ok) {
-      const float2 xk = src[k], xm = src[M - k];
+      float2 xk = src[k], xm = src[M - k];
+      if (gz) {   // fused gradient along z: g(w_z) with g(0) = g(Nyquist) = 0
+        const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
+        xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
+      }
       if (k == 0) {
         z = make_float2(xk.x + xm.x, xk.x - xm.x);
       } else {

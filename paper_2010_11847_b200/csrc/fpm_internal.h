@@ -13,7 +13,7 @@ namespace fpm {
 // ---- per-kernel accounting: launch counter (always) + CUDA-event timing (when enabled) --------
 enum KernelId {
   K_PAINT = 0, K_FFT_Z_R2C, K_FFT_Y, K_FFT_X, K_FFT_Z_C2R, K_GREEN, K_READOUT, K_READOUT_KICK_DRIFT,
-  K_KICK, K_DRIFT, K_READOUT_GRAD, K_LPT, K_COUNT
+  K_KICK, K_DRIFT, K_READOUT_GRAD, K_LPT, K_FFT_X_FORCE, K_FFT_Y_INV3, K_MEMSET, K_COUNT
 };
 const char* kernel_name(int kid);
 
@@ -73,13 +73,25 @@ cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStr
 cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s,
                     Profiler* prof = nullptr);
 
+// paint'ed density -> the three force meshes F[0..2] with the transfer function fused into the
+// transform passes (fft.cu); scale = 1.5 omega_m (or 1)
+cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
+                            float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                            cudaStream_t s, Profiler* prof = nullptr);
+
 // ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
+// How the caller's particle arrays are ordered: np > 0 says "n == np^3 particles in lattice
+// (Lagrangian) order", which lets the kernels walk them brick by brick; results never depend on it.
+struct ParticleOrder {
+  int np = 0;
+  int paint_mode = FPM_PAINT_AUTO;
+};
 cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
-                  float* mesh, bool zero_first, cudaStream_t s);
+                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s);
 cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, float* out,
-                    cudaStream_t s);
+                    const ParticleOrder& ord, cudaStream_t s);
 cudaError_t readout3(const float* fx, const float* fy, const float* fz, const float* pos, int64_t n,
-                     int ng, float* out3, cudaStream_t s);
+                     int ng, float* out3, const ParticleOrder& ord, cudaStream_t s);
 // gradient of the CIC sum w.r.t. the position, times scale_p (mass[p] or vbar[p] or constant)
 cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale, float scale_const,
                          int64_t n, int ng, float* out3, float* out_value, cudaStream_t s);
@@ -90,7 +102,7 @@ cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, c
 // mom += force(pos) * kfac ; pos = wrap(pos + mom * dfac), gathering the three force meshes
 cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
                                float* mom, int64_t n, int ng, float kfac, float dfac,
-                               cudaStream_t s);
+                               const ParticleOrder& ord, cudaStream_t s);
 
 // ---- transfer function and LPT element-wise kernels (green.cu) ---------------------------------
 cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float scale, float2* fkx,

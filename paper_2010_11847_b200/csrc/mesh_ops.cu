@@ -1,6 +1,18 @@
 // mesh_ops.cu -- cloud-in-cell paint (scatter), readout (gather) and their position gradients.
 // PAPER.md:47 "linear window of unit size corresponding to the cloud-in-cell (CIC) interpolation
 // scheme"; PAPER.md:51 readout "with the same kernel"; adjoints per SURVEY.md 8(c) R11.
+//
+// sm_100a design:
+//   * Particles of a run are stored in Lagrangian (lattice) order and move a few cells at most, so a
+//     brick of 8 x 16 x 32 lattice neighbours stays a compact Eulerian cloud.  One CTA owns one
+//     brick.  Readout: the brick's gathers hit the same few mesh rows, which therefore stay in that
+//     SM's L1; bricks are scheduled in memory order so the mesh streams through L2 exactly once.
+//   * Paint: global fp32 reductions are bounded by the L2 atomic units (measured ~0.6 T RED/s, 8 per
+//     particle), so the brick accumulates into a shared-memory window placed at its mean
+//     displacement and flushes the window with one 16-byte vector reduction per 4 cells
+//     (RED.E.ADD.F32x4); the few particles outside the window fall back to direct reductions.
+//     Shared memory has no native fp32 add (ATOMS.CAST.SPIN loop), so the window accumulates in
+//     32-bit fixed point with a per-brick scale that cannot overflow (native ATOMS.ADD).
 #include "fpm_internal.h"
 
 namespace fpm {
@@ -34,64 +46,284 @@ __device__ __forceinline__ float ld_stream(const float* p) {
 
 constexpr int kThreads = 256;
 
-// Baseline scatter: one thread per particle, 8 fp32 reductions (RED.ADD.F32) into L2.
+// ---- Lagrangian bricks ------------------------------------------------------------------------
+// Brick = BX x BY x BZ neighbouring lattice sites (z fastest, one warp = one 128-byte z run).
+constexpr int BX = 8, BY = 16, BZ = 32;
+constexpr int kBrick = BX * BY * BZ;          // 4096 particles
+constexpr int kBrickThreads = 512;
+constexpr int kPerThread = kBrick / kBrickThreads;
+
+struct BrickMap {
+  int np, nbz, nby;
+  __device__ __forceinline__ void origin(int64_t bid, int& qx0, int& qy0, int& qz0) const {
+    const int bz = (int)(bid % nbz);
+    const int64_t r = bid / nbz;
+    qz0 = bz * BZ;
+    qy0 = (int)(r % nby) * BY;
+    qx0 = (int)(r / nby) * BX;
+  }
+  // particle index of slot s (0 .. kBrick-1) of the brick with lattice origin (qx0, qy0, qz0)
+  __device__ __forceinline__ int64_t index(int qx0, int qy0, int qz0, int s) const {
+    const int lz = s & (BZ - 1), ly = (s >> 5) & (BY - 1), lx = s >> 9;
+    return ((int64_t)(qx0 + lx) * np + (qy0 + ly)) * np + (qz0 + lz);
+  }
+};
+
+inline bool brick_ok(int64_t n, int np) {
+  return np >= 32 && np % 32 == 0 && n == (int64_t)np * np * np;
+}
+
+// ---- paint: direct reductions --------------------------------------------------------------------
+__device__ __forceinline__ void deposit_global(float* __restrict__ mesh, int64_t g, const Cic& c,
+                                               float m) {
+  const float wx[2] = {m * (1.f - c.t[0]), m * c.t[0]};
+  const float wy[2] = {1.f - c.t[1], c.t[1]};
+  const float wz[2] = {1.f - c.t[2], c.t[2]};
+  const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]};
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      float* row = mesh + ((int64_t)ix[a] * g + iy[b]) * g;
+      const float w = wx[a] * wy[b];
+      atomicAdd(row + c.i0[2], w * wz[0]);
+      atomicAdd(row + c.i1[2], w * wz[1]);
+    }
+}
+
+// One thread per particle in memory order, 8 fp32 reductions (RED.ADD.F32) into L2.  Blocks are
+// contiguous chunks so the touched mesh rows form a sliding window that stays in L2.
 __global__ void __launch_bounds__(kThreads)
-paint_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
-             int64_t n, int ng, float* __restrict__ mesh) {
+paint_direct_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
+                    int64_t n, int ng, float* __restrict__ mesh) {
+  const int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  if (p >= n) return;
+  const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), ng - 1);
+  deposit_global(mesh, ng, c, mass ? ld_stream(mass + p) : mass_const);
+}
+
+// ---- paint: brick window in shared memory ----------------------------------------------------------
+// Window of the brick (resolution factor 1): brick extent + kHalo cells either side + 1 (CIC reaches
+// the next cell); z is padded so the origin can be rounded down to a multiple of 4 cells.
+constexpr int kHalo = 4;
+constexpr int WX = BX + 2 * kHalo + 1, WY = BY + 2 * kHalo + 1;
+constexpr int WZ = (BZ + 2 * kHalo + 1 + 3 + 3) & ~3;
+constexpr int kWinCells = WX * WY * WZ;       // 17 x 25 x 44 = 18700 cells, 74.8 KB
+
+template <bool FIXED, bool HAS_MASS>
+__global__ void __launch_bounds__(kBrickThreads, 2)
+paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
+                   int64_t n, BrickMap bm, int ng, float* __restrict__ mesh) {
+  extern __shared__ __align__(16) float win_f[];
+  int* win_i = reinterpret_cast<int*>(win_f);
+  __shared__ float red[4][kBrickThreads / 32];
   const int mask = ng - 1;
-  const int64_t g = ng;
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n;
-       p += (int64_t)gridDim.x * blockDim.x) {
-    const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), mask);
-    const float m = mass ? ld_stream(mass + p) : mass_const;
-    const float wx[2] = {m * (1.f - c.t[0]), m * c.t[0]};
-    const float wy[2] = {1.f - c.t[1], c.t[1]};
-    const float wz[2] = {1.f - c.t[2], c.t[2]};
-    const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]}, iz[2] = {c.i0[2], c.i1[2]};
+  const float fng = (float)ng, inv_ng = 1.f / fng;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  int qx0, qy0, qz0;
+  bm.origin(blockIdx.x, qx0, qy0, qz0);
+
+  for (int i = tid; i < kWinCells / 4; i += kBrickThreads)
+    reinterpret_cast<float4*>(win_f)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+
+  // this thread's particles (slot s = tid + 512 k: lattice offsets lz = lane, ly = warp, lx = k)
+  float x[kPerThread], y[kPerThread], z[kPerThread], m[HAS_MASS ? kPerThread : 1];
+  const int64_t p0 = bm.index(qx0, qy0, qz0, tid);
+  const int64_t plane = (int64_t)bm.np * bm.np;
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
+  for (int k = 0; k < kPerThread; ++k) {
+    const int64_t p = p0 + k * plane;
+    x[k] = ld_stream(pos + p);
+    y[k] = ld_stream(pos + n + p);
+    z[k] = ld_stream(pos + 2 * n + p);
+    if (HAS_MASS) m[k] = ld_stream(mass + p);
+  }
+  // mean displacement from the lattice sites (wrapped to [-ng/2, ng/2)) places the window
+  float sx = 0.f, sy = 0.f, sz = 0.f, mmax = HAS_MASS ? 0.f : fabsf(mass_const);
+  const float qy = (float)(qy0 + warp), qz = (float)(qz0 + lane);
 #pragma unroll
-      for (int b = 0; b < 2; ++b) {
-        float* row = mesh + ((int64_t)ix[a] * g + iy[b]) * g;
-        const float w = wx[a] * wy[b];
-        atomicAdd(row + iz[0], w * wz[0]);
-        atomicAdd(row + iz[1], w * wz[1]);
+  for (int k = 0; k < kPerThread; ++k) {
+    float dx = x[k] - (float)(qx0 + k), dy = y[k] - qy, dz = z[k] - qz;
+    dx -= fng * rintf(dx * inv_ng);
+    dy -= fng * rintf(dy * inv_ng);
+    dz -= fng * rintf(dz * inv_ng);
+    sx += dx; sy += dy; sz += dz;
+    if (HAS_MASS) mmax = fmaxf(mmax, fabsf(m[k]));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sx += __shfl_xor_sync(0xffffffffu, sx, o);
+    sy += __shfl_xor_sync(0xffffffffu, sy, o);
+    sz += __shfl_xor_sync(0xffffffffu, sz, o);
+    if (HAS_MASS) mmax = fmaxf(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
+  }
+  if (lane == 0) { red[0][warp] = sx; red[1][warp] = sy; red[2][warp] = sz; red[3][warp] = mmax; }
+  __syncthreads();   // also orders the window zeroing before the deposits
+  sx = sy = sz = 0.f;
+#pragma unroll
+  for (int i = 0; i < kBrickThreads / 32; ++i) {
+    sx += red[0][i]; sy += red[1][i]; sz += red[2][i];
+    if (HAS_MASS) mmax = fmaxf(mmax, red[3][i]);
+  }
+  constexpr float inv_cnt = 1.f / (float)kBrick;
+  const int ox = qx0 + (int)floorf(sx * inv_cnt) - kHalo;
+  const int oy = qy0 + (int)floorf(sy * inv_cnt) - kHalo;
+  const int oz = (qz0 + (int)floorf(sz * inv_cnt) - kHalo) & ~3;
+  // Fixed point with a power-of-two scale (exact for weights that are dyadic fractions).  No cell can
+  // overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2) <= 2^30 + 2^11 < 2^31.
+  const float scale = FIXED ? (mmax > 0.f ? ldexpf(1.f, ilogbf((float)(1 << 18) / mmax)) : 0.f) : 1.f;
+
+#pragma unroll
+  for (int k = 0; k < kPerThread; ++k) {
+    const float fx = floorf(x[k]), fy = floorf(y[k]), fz = floorf(z[k]);
+    const float tx = x[k] - fx, ty = y[k] - fy, tz = z[k] - fz;
+    const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+    const unsigned rx = (ix - ox) & mask, ry = (iy - oy) & mask, rz = (iz - oz) & mask;
+    const float mk = HAS_MASS ? m[k] : mass_const;
+    if (rx < WX - 1 && ry < WY - 1 && rz < WZ - 1) {
+      const float mm = mk * scale;
+      const float w00 = mm * (1.f - tx) * (1.f - ty), w01 = mm * (1.f - tx) * ty;
+      const float w10 = mm * tx * (1.f - ty), w11 = mm * tx * ty;
+      const float wz0 = 1.f - tz, wz1 = tz;
+      const int base = (rx * WY + ry) * WZ + rz;
+      if (FIXED) {
+        int* c = win_i + base;
+        atomicAdd(c, __float2int_rn(w00 * wz0));
+        atomicAdd(c + 1, __float2int_rn(w00 * wz1));
+        atomicAdd(c + WZ, __float2int_rn(w01 * wz0));
+        atomicAdd(c + WZ + 1, __float2int_rn(w01 * wz1));
+        atomicAdd(c + WY * WZ, __float2int_rn(w10 * wz0));
+        atomicAdd(c + WY * WZ + 1, __float2int_rn(w10 * wz1));
+        atomicAdd(c + WY * WZ + WZ, __float2int_rn(w11 * wz0));
+        atomicAdd(c + WY * WZ + WZ + 1, __float2int_rn(w11 * wz1));
+      } else {
+        float* c = win_f + base;
+        atomicAdd(c, w00 * wz0);
+        atomicAdd(c + 1, w00 * wz1);
+        atomicAdd(c + WZ, w01 * wz0);
+        atomicAdd(c + WZ + 1, w01 * wz1);
+        atomicAdd(c + WY * WZ, w10 * wz0);
+        atomicAdd(c + WY * WZ + 1, w10 * wz1);
+        atomicAdd(c + WY * WZ + WZ, w11 * wz0);
+        atomicAdd(c + WY * WZ + WZ + 1, w11 * wz1);
       }
+    } else {
+      Cic c;
+      c.t[0] = tx; c.t[1] = ty; c.t[2] = tz;
+      c.i0[0] = ix & mask; c.i1[0] = (ix + 1) & mask;
+      c.i0[1] = iy & mask; c.i1[1] = (iy + 1) & mask;
+      c.i0[2] = iz & mask; c.i1[2] = (iz + 1) & mask;
+      deposit_global(mesh, ng, c, mk);
+    }
+  }
+  __syncthreads();
+
+  // flush: one 16-byte vector reduction per 4 z-cells (oz and ng are multiples of 4)
+  const float inv_scale = FIXED ? (scale > 0.f ? 1.f / scale : 0.f) : 1.f;
+  constexpr int WZ4 = WZ / 4;
+  for (int gidx = tid; gidx < kWinCells / 4; gidx += kBrickThreads) {
+    float4 v;
+    if (FIXED) {
+      const int4 q = reinterpret_cast<const int4*>(win_i)[gidx];
+      if ((q.x | q.y | q.z | q.w) == 0) continue;
+      v = make_float4(q.x * inv_scale, q.y * inv_scale, q.z * inv_scale, q.w * inv_scale);
+    } else {
+      v = reinterpret_cast<const float4*>(win_f)[gidx];
+      if (v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f) continue;
+    }
+    const int kz = gidx % WZ4, r = gidx / WZ4;
+    const int ky = r % WY, kx = r / WY;
+    const int gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
+    atomicAdd(reinterpret_cast<float4*>(mesh + ((int64_t)gx * ng + gy) * ng + gz), v);
   }
 }
 
+// ---- readout -----------------------------------------------------------------------------------
 template <int NMESH>
-__global__ void __launch_bounds__(kThreads)
+__device__ __forceinline__ void gather(const float* const* mesh, const Cic& c, int64_t g,
+                                       float (&acc)[NMESH]) {
+  const float wx[2] = {1.f - c.t[0], c.t[0]};
+  const float wy[2] = {1.f - c.t[1], c.t[1]};
+  const float wz[2] = {1.f - c.t[2], c.t[2]};
+  const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]};
+#pragma unroll
+  for (int k = 0; k < NMESH; ++k) acc[k] = 0.f;
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
+      const float w = wx[a] * wy[b];
+#pragma unroll
+      for (int k = 0; k < NMESH; ++k) {
+        acc[k] = fmaf(__ldg(mesh[k] + row + c.i0[2]), w * wz[0], acc[k]);
+        acc[k] = fmaf(__ldg(mesh[k] + row + c.i1[2]), w * wz[1], acc[k]);
+      }
+    }
+}
+
+// particle handled by (block, thread, k): brick order when bm.np > 0, memory order otherwise
+template <int NMESH, bool BRICK>
+__global__ void __launch_bounds__(BRICK ? kBrickThreads : kThreads)
 readout_kernel(const float* __restrict__ m0, const float* __restrict__ m1,
                const float* __restrict__ m2, const float* __restrict__ pos, int64_t n, int ng,
-               float* __restrict__ out) {
-  const int mask = ng - 1;
-  const int64_t g = ng;
-  const float* mesh[3] = {m0, m1, m2};
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n;
-       p += (int64_t)gridDim.x * blockDim.x) {
-    const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), mask);
-    const float wx[2] = {1.f - c.t[0], c.t[0]};
-    const float wy[2] = {1.f - c.t[1], c.t[1]};
-    const float wz[2] = {1.f - c.t[2], c.t[2]};
-    const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]}, iz[2] = {c.i0[2], c.i1[2]};
+               BrickMap bm, float* __restrict__ out) {
+  const float* const mesh3[3] = {m0, m1, m2};
+  const float* meshn[NMESH];
+#pragma unroll
+  for (int j = 0; j < NMESH; ++j) meshn[j] = mesh3[j];
+  int qx0 = 0, qy0 = 0, qz0 = 0;
+  if (BRICK) bm.origin(blockIdx.x, qx0, qy0, qz0);
+  constexpr int K = BRICK ? kPerThread : 1;
+#pragma unroll 2
+  for (int k = 0; k < K; ++k) {
+    int64_t p;
+    if (BRICK) p = bm.index(qx0, qy0, qz0, threadIdx.x + k * kBrickThreads);
+    else { p = (int64_t)blockIdx.x * kThreads + threadIdx.x; if (p >= n) return; }
+    const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), ng - 1);
     float acc[NMESH];
+    gather<NMESH>(meshn, c, ng, acc);
 #pragma unroll
-    for (int k = 0; k < NMESH; ++k) acc[k] = 0.f;
+    for (int j = 0; j < NMESH; ++j) out[j * n + p] = acc[j];
+  }
+}
+
+__device__ __forceinline__ float wrap_box(float x, float ng, float inv_ng) {
+  x -= ng * floorf(x * inv_ng);
+  if (x >= ng) x -= ng;
+  if (x < 0.f) x += ng;
+  return x >= ng ? 0.f : x;
+}
+
+// One pass over the particles: gather the three force components at x (CIC),
+// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).
+template <bool BRICK>
+__global__ void __launch_bounds__(BRICK ? kBrickThreads : kThreads)
+readout_kick_drift_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
+                          const float* __restrict__ fz, float* __restrict__ pos,
+                          float* __restrict__ mom, int64_t n, int ngi, BrickMap bm, float kfac,
+                          float dfac) {
+  const float ng = (float)ngi, inv_ng = 1.f / ng;
+  const float* const mesh[3] = {fx, fy, fz};
+  int qx0 = 0, qy0 = 0, qz0 = 0;
+  if (BRICK) bm.origin(blockIdx.x, qx0, qy0, qz0);
+  constexpr int K = BRICK ? kPerThread : 1;
+#pragma unroll 2
+  for (int k = 0; k < K; ++k) {
+    int64_t p;
+    if (BRICK) p = bm.index(qx0, qy0, qz0, threadIdx.x + k * kBrickThreads);
+    else { p = (int64_t)blockIdx.x * kThreads + threadIdx.x; if (p >= n) return; }
+    const float x[3] = {ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p)};
+    const float m[3] = {ld_stream(mom + p), ld_stream(mom + n + p), ld_stream(mom + 2 * n + p)};
+    const Cic c = cic_of(x[0], x[1], x[2], ngi - 1);
+    float acc[3];
+    gather<3>(mesh, c, ngi, acc);
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
-#pragma unroll
-      for (int b = 0; b < 2; ++b) {
-        const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
-        const float w = wx[a] * wy[b];
-#pragma unroll
-        for (int k = 0; k < NMESH; ++k) {
-          acc[k] = fmaf(__ldg(mesh[k] + row + iz[0]), w * wz[0], acc[k]);
-          acc[k] = fmaf(__ldg(mesh[k] + row + iz[1]), w * wz[1], acc[k]);
-        }
-      }
-#pragma unroll
-    for (int k = 0; k < NMESH; ++k) out[k * n + p] = acc[k];
+    for (int d = 0; d < 3; ++d) {
+      const float mn = fmaf(acc[d], kfac, m[d]);
+      __stcs(mom + d * n + p, mn);
+      __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[d]), ng, inv_ng));
+    }
   }
 }
 
@@ -100,79 +332,114 @@ __global__ void __launch_bounds__(kThreads)
 readout_grad_kernel(const float* __restrict__ mesh, const float* __restrict__ pos,
                     const float* __restrict__ scale, float scale_const, int64_t n, int ng,
                     float* __restrict__ out3, float* __restrict__ out_value) {
-  const int mask = ng - 1;
   const int64_t g = ng;
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n;
-       p += (int64_t)gridDim.x * blockDim.x) {
-    const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), mask);
-    const float wx[2] = {1.f - c.t[0], c.t[0]};
-    const float wy[2] = {1.f - c.t[1], c.t[1]};
-    const float wz[2] = {1.f - c.t[2], c.t[2]};
-    const float sg[2] = {-1.f, 1.f};
-    const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]}, iz[2] = {c.i0[2], c.i1[2]};
-    float gx = 0.f, gy = 0.f, gz = 0.f, val = 0.f;
+  const int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  if (p >= n) return;
+  const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), ng - 1);
+  const float wx[2] = {1.f - c.t[0], c.t[0]};
+  const float wy[2] = {1.f - c.t[1], c.t[1]};
+  const float wz[2] = {1.f - c.t[2], c.t[2]};
+  const float sg[2] = {-1.f, 1.f};
+  const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]}, iz[2] = {c.i0[2], c.i1[2]};
+  float gx = 0.f, gy = 0.f, gz = 0.f, val = 0.f;
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
+  for (int a = 0; a < 2; ++a)
 #pragma unroll
-      for (int b = 0; b < 2; ++b) {
-        const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
+    for (int b = 0; b < 2; ++b) {
+      const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const float v = __ldg(mesh + row + iz[e]);
-          gx = fmaf(v, sg[a] * wy[b] * wz[e], gx);
-          gy = fmaf(v, wx[a] * sg[b] * wz[e], gy);
-          gz = fmaf(v, wx[a] * wy[b] * sg[e], gz);
-          val = fmaf(v, wx[a] * wy[b] * wz[e], val);
-        }
+      for (int e = 0; e < 2; ++e) {
+        const float v = __ldg(mesh + row + iz[e]);
+        gx = fmaf(v, sg[a] * wy[b] * wz[e], gx);
+        gy = fmaf(v, wx[a] * sg[b] * wz[e], gy);
+        gz = fmaf(v, wx[a] * wy[b] * sg[e], gz);
+        val = fmaf(v, wx[a] * wy[b] * wz[e], val);
       }
-    const float s = scale ? ld_stream(scale + p) : scale_const;
-    out3[p] = s * gx;
-    out3[n + p] = s * gy;
-    out3[2 * n + p] = s * gz;
-    if (out_value) out_value[p] = val;
-  }
+    }
+  const float s = scale ? ld_stream(scale + p) : scale_const;
+  out3[p] = s * gx;
+  out3[n + p] = s * gy;
+  out3[2 * n + p] = s * gz;
+  if (out_value) out_value[p] = val;
 }
 
-inline unsigned grid_for(int64_t n) {
-  int64_t b = (n + kThreads - 1) / kThreads;
-  const int64_t cap = 148LL * 64;   // grid-stride beyond 64 waves of CTAs per SM
-  if (b > cap) b = cap;
-  if (b < 1) b = 1;
-  return (unsigned)b;
-}
+inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kThreads - 1) / kThreads); }
+
+inline BrickMap brick_map(int np) { return BrickMap{np, np / BZ, np / BY}; }
 
 }  // namespace
 
 cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
-                  float* mesh, bool zero_first, cudaStream_t s) {
+                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s) {
   if (zero_first) {
     cudaError_t e = cudaMemsetAsync(mesh, 0, sizeof(float) * (size_t)ng * ng * ng, s);
     if (e != cudaSuccess) return e;
   }
   if (n == 0) return cudaSuccess;
-  paint_kernel<<<grid_for(n), kThreads, 0, s>>>(pos, mass, mass_const, n, ng, mesh);
-  return cudaGetLastError();
+  int mode = ord.paint_mode;
+  const bool can_brick = brick_ok(n, ord.np) && ng == ord.np && ng % 4 == 0 &&
+                         (reinterpret_cast<uintptr_t>(mesh) & 15) == 0;
+  if (mode == FPM_PAINT_AUTO) mode = can_brick ? FPM_PAINT_BRICK_FIXED : FPM_PAINT_DIRECT;
+  if (mode != FPM_PAINT_DIRECT && !can_brick) mode = FPM_PAINT_DIRECT;
+  if (mode == FPM_PAINT_DIRECT) {
+    paint_direct_kernel<<<blocks_for(n), kThreads, 0, s>>>(pos, mass, mass_const, n, ng, mesh);
+    return cudaGetLastError();
+  }
+  const size_t smem = sizeof(float) * (size_t)kWinCells;
+  const unsigned grid = (unsigned)(n / kBrick);
+  const BrickMap bm = brick_map(ord.np);
+  auto go = [&](auto kern) -> cudaError_t {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kBrickThreads, smem, s>>>(pos, mass, mass_const, n, bm, ng, mesh);
+    return cudaGetLastError();
+  };
+  if (mode == FPM_PAINT_BRICK_FIXED)
+    return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
+  return mass ? go(paint_brick_kernel<false, true>) : go(paint_brick_kernel<false, false>);
 }
 
 cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, float* out,
-                    cudaStream_t s) {
+                    const ParticleOrder& ord, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  readout_kernel<1><<<grid_for(n), kThreads, 0, s>>>(mesh, nullptr, nullptr, pos, n, ng, out);
+  if (brick_ok(n, ord.np))
+    readout_kernel<1, true><<<(unsigned)(n / kBrick), kBrickThreads, 0, s>>>(mesh, nullptr, nullptr, pos, n, ng,
+                                                                           brick_map(ord.np), out);
+  else
+    readout_kernel<1, false><<<blocks_for(n), kThreads, 0, s>>>(mesh, nullptr, nullptr, pos, n, ng,
+                                                               BrickMap{0, 1, 1}, out);
   return cudaGetLastError();
 }
 
 cudaError_t readout3(const float* fx, const float* fy, const float* fz, const float* pos, int64_t n,
-                     int ng, float* out3, cudaStream_t s) {
+                     int ng, float* out3, const ParticleOrder& ord, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  readout_kernel<3><<<grid_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, n, ng, out3);
+  if (brick_ok(n, ord.np))
+    readout_kernel<3, true><<<(unsigned)(n / kBrick), kBrickThreads, 0, s>>>(fx, fy, fz, pos, n, ng,
+                                                                           brick_map(ord.np), out3);
+  else
+    readout_kernel<3, false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, n, ng, BrickMap{0, 1, 1}, out3);
+  return cudaGetLastError();
+}
+
+cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
+                               float* mom, int64_t n, int ng, float kfac, float dfac,
+                               const ParticleOrder& ord, cudaStream_t s) {
+  if (n == 0) return cudaSuccess;
+  if (brick_ok(n, ord.np))
+    readout_kick_drift_kernel<true><<<(unsigned)(n / kBrick), kBrickThreads, 0, s>>>(
+        fx, fy, fz, pos, mom, n, ng, brick_map(ord.np), kfac, dfac);
+  else
+    readout_kick_drift_kernel<false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng,
+                                                                       BrickMap{0, 1, 1}, kfac, dfac);
   return cudaGetLastError();
 }
 
 cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale, float scale_const,
                          int64_t n, int ng, float* out3, float* out_value, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  readout_grad_kernel<<<grid_for(n), kThreads, 0, s>>>(mesh, pos, scale, scale_const, n, ng, out3,
-                                                       out_value);
+  readout_grad_kernel<<<blocks_for(n), kThreads, 0, s>>>(mesh, pos, scale, scale_const, n, ng, out3,
+                                                         out_value);
   return cudaGetLastError();
 }
 

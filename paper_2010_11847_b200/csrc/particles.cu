@@ -1,5 +1,5 @@
-// particles.cu -- kick and drift (Eq. 1-2) as streaming passes, and the fused
-// readout + kick + drift pass used by the whole-run driver.
+// particles.cu -- kick and drift (Eq. 1-2) as streaming passes (the fused
+// readout + kick + drift pass of the whole-run driver lives in mesh_ops.cu).
 #include "fpm_internal.h"
 
 namespace fpm {
@@ -69,52 +69,6 @@ drift_scalar_kernel(float* __restrict__ pos, const float* __restrict__ mom, int6
     pos[i] = wrap_box(fmaf(mom[i], fac, pos[i]), ng, inv_ng);
 }
 
-// One pass over the particles: gather the three force components at x (CIC),
-// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).
-__global__ void __launch_bounds__(kThreads)
-readout_kick_drift_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
-                          const float* __restrict__ fz, float* __restrict__ pos,
-                          float* __restrict__ mom, int64_t n, int ngi, float kfac, float dfac) {
-  const int mask = ngi - 1;
-  const int64_t g = ngi;
-  const float ng = (float)ngi, inv_ng = 1.f / ng;
-  const float* mesh[3] = {fx, fy, fz};
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n;
-       p += (int64_t)gridDim.x * blockDim.x) {
-    float x[3] = {pos[p], pos[n + p], pos[2 * n + p]};
-    int i0[3], i1[3];
-    float t[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const float fl = floorf(x[d]);
-      t[d] = x[d] - fl;
-      i0[d] = (int)fl & mask;
-      i1[d] = ((int)fl + 1) & mask;
-    }
-    const float wx[2] = {1.f - t[0], t[0]}, wy[2] = {1.f - t[1], t[1]}, wz[2] = {1.f - t[2], t[2]};
-    const int ix[2] = {i0[0], i1[0]}, iy[2] = {i0[1], i1[1]}, iz[2] = {i0[2], i1[2]};
-    float acc[3] = {0.f, 0.f, 0.f};
-#pragma unroll
-    for (int a = 0; a < 2; ++a)
-#pragma unroll
-      for (int b = 0; b < 2; ++b) {
-        const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
-        const float w = wx[a] * wy[b];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-          acc[k] = fmaf(__ldg(mesh[k] + row + iz[0]), w * wz[0], acc[k]);
-          acc[k] = fmaf(__ldg(mesh[k] + row + iz[1]), w * wz[1], acc[k]);
-        }
-      }
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const float m = fmaf(acc[d], kfac, mom[d * n + p]);
-      mom[d * n + p] = m;
-      pos[d * n + p] = wrap_box(fmaf(m, dfac, x[d]), ng, inv_ng);
-    }
-  }
-}
-
 inline unsigned grid_for(int64_t n) {
   int64_t b = (n + kThreads - 1) / kThreads;
   const int64_t cap = 148LL * 64;
@@ -142,14 +96,6 @@ cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, c
     drift_kernel<<<grid_for(n3 / 4 + 1), kThreads, 0, s>>>(pos, mom, n3, fac, (float)ng, 1.f / ng);
   else
     drift_scalar_kernel<<<grid_for(n3), kThreads, 0, s>>>(pos, mom, n3, fac, (float)ng, 1.f / ng);
-  return cudaGetLastError();
-}
-
-cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
-                               float* mom, int64_t n, int ng, float kfac, float dfac,
-                               cudaStream_t s) {
-  if (n == 0) return cudaSuccess;
-  readout_kick_drift_kernel<<<grid_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, kfac, dfac);
   return cudaGetLastError();
 }
 

@@ -37,7 +37,7 @@ def test_argument_validation_needs_no_gpu():
         _fields_ = [("ng", ctypes.c_int32), ("np", ctypes.c_int32), ("omega_m", ctypes.c_double),
                     ("box", ctypes.c_double), ("kernel_mode", ctypes.c_int32),
                     ("factor_mode", ctypes.c_int32), ("force_path", ctypes.c_int32),
-                    ("reserved", ctypes.c_int32)]
+                    ("paint_mode", ctypes.c_int32)]
 
     lib.fpm_workspace_bytes.restype = ctypes.c_size_t
     good = Cfg(512, 512, 0.3075, 1000.0, 0, 0, 0, 0)

@@ -47,12 +47,14 @@ def test_growth_and_factors_match_oracle(fpm, oracle):
     assert cq.kick_factor(0.1, 0.2, 0.3) == pytest.approx(oracle.kick_factor(OM, 0.1, 0.2, 0.3, 1), rel=1e-9)
 
 
-@pytest.mark.parametrize("ng,nps,mode", [(32, 32, 0), (64, 32, 0), (64, 64, 1), (128, 128, 0)])
-def test_force_evaluation_matches_oracle(fpm, oracle, ng, nps, mode):
-    """paint -> r2c -> kernel -> 3 c2r -> readout at a clustered (a ~ 1-like) particle set."""
+@pytest.mark.parametrize("force_path", [0, 1])
+@pytest.mark.parametrize("ng,nps,mode", [(32, 32, 0), (64, 32, 0), (64, 64, 1), (64, 64, 2), (128, 128, 0)])
+def test_force_evaluation_matches_oracle(fpm, oracle, ng, nps, mode, force_path):
+    """paint -> r2c -> kernel -> 3 c2r -> readout at a clustered (a ~ 1-like) particle set, with the
+    transfer function as its own kernel (force_path 0) and fused into the FFT passes (1)."""
     n = nps ** 3
     pos = fi.random_particles(n, ng, seed=ng + mode, clustered=True)
-    ctx = fpm.FPM(ng, nps, kernel_mode=mode)
+    ctx = fpm.FPM(ng, nps, kernel_mode=mode, force_path=force_path)
     got = host(ctx.force(dev(pos)))
     ref, rho = oracle.force(pos.astype(np.float64), ng, mode=mode, scale=1.5 * OM,
                             mass=float((ng // nps) ** 3), return_rho=True)
