@@ -45,7 +45,7 @@ def test_argument_validation_needs_no_gpu():
     assert lib.fpm_workspace_bytes(ctypes.byref(good)) == 4 * 512 ** 3 * 4 + 4 * nk * 8
     for bad in (Cfg(500, 500, 0.3, 0, 0, 0, 0, 0), Cfg(64, 128, 0.3, 0, 0, 0, 0, 0),
                 Cfg(2048, 2048, 0.3, 0, 0, 0, 0, 0), Cfg(64, 64, -1.0, 0, 0, 0, 0, 0),
-                Cfg(64, 64, 0.3, 0, 7, 0, 0, 0), Cfg(64, 64, 0.3, 0, 0, 0, 0, 1)):
+                Cfg(64, 64, 0.3, 0, 7, 0, 0, 0), Cfg(64, 64, 0.3, 0, 0, 0, 0, 9), Cfg(64, 64, 0.3, 0, 0, 0, 5, 0)):
         assert lib.fpm_workspace_bytes(ctypes.byref(bad)) == 0
         h = ctypes.c_void_p()
         assert lib.fpm_create(ctypes.byref(bad), None, ctypes.byref(h)) == -1
