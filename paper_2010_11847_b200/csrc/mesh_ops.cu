@@ -24,14 +24,31 @@ struct Cic {
   float t[3];
 };
 
+// floor / round-to-nearest without the conversion (XU) pipe: adding 1.5 * 2^23 leaves the integer in
+// the low mantissa bits.  Exact for |x| < 2^22, far beyond any position in mesh cells (ng <= 1024);
+// FRND/F2I issue at a quarter of the FMA rate and dominated the paint kernel (profiles/r01_A).
+constexpr float kMagic = 12582912.f;
+constexpr int kMagicBits = 0x4B400000;
+__device__ __forceinline__ float fast_rint(float x, int& i) {
+  const float t = x + kMagic;
+  i = __float_as_int(t) - kMagicBits;
+  return t - kMagic;
+}
+__device__ __forceinline__ float fast_floor(float x, int& i) {
+  float r = fast_rint(x, i);
+  if (r > x) { r -= 1.f; i -= 1; }
+  return r;
+}
+__device__ __forceinline__ int fast_round_to_int(float x) { return __float_as_int(x + kMagic) - kMagicBits; }
+
 __device__ __forceinline__ Cic cic_of(float x, float y, float z, int mask) {
   Cic c;
   const float p[3] = {x, y, z};
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    const float fl = floorf(p[d]);
+    int i;
+    const float fl = fast_floor(p[d], i);
     c.t[d] = p[d] - fl;
-    const int i = (int)fl;
     c.i0[d] = i & mask;
     c.i1[d] = (i + 1) & mask;
   }
@@ -41,6 +58,13 @@ __device__ __forceinline__ Cic cic_of(float x, float y, float z, int mask) {
 __device__ __forceinline__ float ld_stream(const float* p) {
   float v;
   asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+
+// same, for arrays the kernel updates in place (no .nc; ordered against the later stores)
+__device__ __forceinline__ float ld_stream_rw(const float* p) {
+  float v;
+  asm volatile("ld.global.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
   return v;
 }
 
@@ -144,9 +168,10 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
     float dx = x[k] - (float)(qx0 + k), dy = y[k] - qy, dz = z[k] - qz;
-    dx -= fng * rintf(dx * inv_ng);
-    dy -= fng * rintf(dy * inv_ng);
-    dz -= fng * rintf(dz * inv_ng);
+    int unused;
+    dx -= fng * fast_rint(dx * inv_ng, unused);
+    dy -= fng * fast_rint(dy * inv_ng, unused);
+    dz -= fng * fast_rint(dz * inv_ng, unused);
     sx += dx; sy += dy; sz += dz;
     if (HAS_MASS) mmax = fmaxf(mmax, fabsf(m[k]));
   }
@@ -166,18 +191,24 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
     if (HAS_MASS) mmax = fmaxf(mmax, red[3][i]);
   }
   constexpr float inv_cnt = 1.f / (float)kBrick;
-  const int ox = qx0 + (int)floorf(sx * inv_cnt) - kHalo;
-  const int oy = qy0 + (int)floorf(sy * inv_cnt) - kHalo;
-  const int oz = (qz0 + (int)floorf(sz * inv_cnt) - kHalo) & ~3;
-  // Fixed point with a power-of-two scale (exact for weights that are dyadic fractions).  No cell can
-  // overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2) <= 2^30 + 2^11 < 2^31.
-  const float scale = FIXED ? (mmax > 0.f ? ldexpf(1.f, ilogbf((float)(1 << 18) / mmax)) : 0.f) : 1.f;
+  int mx, my, mz;
+  fast_floor(sx * inv_cnt, mx);
+  fast_floor(sy * inv_cnt, my);
+  fast_floor(sz * inv_cnt, mz);
+  const int ox = qx0 + mx - kHalo;
+  const int oy = qy0 + my - kHalo;
+  const int oz = (qz0 + mz - kHalo) & ~3;
+  // Fixed point with a power-of-two scale 2^floor(log2(2^18 / mmax)) (exact for weights that are dyadic
+  // fractions).  No cell can overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2)
+  // <= 2^30 + 2^11 < 2^31.
+  const float scale = FIXED ? (mmax > 0.f ? __int_as_float(__float_as_int((float)(1 << 18) / mmax) & 0x7F800000) : 0.f)
+                            : 1.f;
 
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
-    const float fx = floorf(x[k]), fy = floorf(y[k]), fz = floorf(z[k]);
+    int ix, iy, iz;
+    const float fx = fast_floor(x[k], ix), fy = fast_floor(y[k], iy), fz = fast_floor(z[k], iz);
     const float tx = x[k] - fx, ty = y[k] - fy, tz = z[k] - fz;
-    const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
     const unsigned rx = (ix - ox) & mask, ry = (iy - oy) & mask, rz = (iz - oz) & mask;
     const float mk = HAS_MASS ? m[k] : mass_const;
     if (rx < WX - 1 && ry < WY - 1 && rz < WZ - 1) {
@@ -188,14 +219,14 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
       const int base = (rx * WY + ry) * WZ + rz;
       if (FIXED) {
         int* c = win_i + base;
-        atomicAdd(c, __float2int_rn(w00 * wz0));
-        atomicAdd(c + 1, __float2int_rn(w00 * wz1));
-        atomicAdd(c + WZ, __float2int_rn(w01 * wz0));
-        atomicAdd(c + WZ + 1, __float2int_rn(w01 * wz1));
-        atomicAdd(c + WY * WZ, __float2int_rn(w10 * wz0));
-        atomicAdd(c + WY * WZ + 1, __float2int_rn(w10 * wz1));
-        atomicAdd(c + WY * WZ + WZ, __float2int_rn(w11 * wz0));
-        atomicAdd(c + WY * WZ + WZ + 1, __float2int_rn(w11 * wz1));
+        atomicAdd(c, fast_round_to_int(w00 * wz0));
+        atomicAdd(c + 1, fast_round_to_int(w00 * wz1));
+        atomicAdd(c + WZ, fast_round_to_int(w01 * wz0));
+        atomicAdd(c + WZ + 1, fast_round_to_int(w01 * wz1));
+        atomicAdd(c + WY * WZ, fast_round_to_int(w10 * wz0));
+        atomicAdd(c + WY * WZ + 1, fast_round_to_int(w10 * wz1));
+        atomicAdd(c + WY * WZ + WZ, fast_round_to_int(w11 * wz0));
+        atomicAdd(c + WY * WZ + WZ + 1, fast_round_to_int(w11 * wz1));
       } else {
         float* c = win_f + base;
         atomicAdd(c, w00 * wz0);
@@ -221,20 +252,29 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   // flush: one 16-byte vector reduction per 4 z-cells (oz and ng are multiples of 4)
   const float inv_scale = FIXED ? (scale > 0.f ? 1.f / scale : 0.f) : 1.f;
   constexpr int WZ4 = WZ / 4;
+  // (kx, ky, kz) of group gidx advance incrementally: no division in the loop
+  constexpr int dKz = kBrickThreads % WZ4, dRow = kBrickThreads / WZ4, dKy = dRow % WY, dKx = dRow / WY;
+  static_assert(kThreads * 2 == kBrickThreads && BX == kPerThread, "half-brick walk of readout_kick_drift");
+  static_assert(dKy + 1 < WY, "one carry per step");
+  int kz = tid % WZ4, ky = (tid / WZ4) % WY, kx = (tid / WZ4) / WY;
   for (int gidx = tid; gidx < kWinCells / 4; gidx += kBrickThreads) {
     float4 v;
+    bool any;
     if (FIXED) {
       const int4 q = reinterpret_cast<const int4*>(win_i)[gidx];
-      if ((q.x | q.y | q.z | q.w) == 0) continue;
+      any = (q.x | q.y | q.z | q.w) != 0;
       v = make_float4(q.x * inv_scale, q.y * inv_scale, q.z * inv_scale, q.w * inv_scale);
     } else {
       v = reinterpret_cast<const float4*>(win_f)[gidx];
-      if (v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f) continue;
+      any = !(v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f);
     }
-    const int kz = gidx % WZ4, r = gidx / WZ4;
-    const int ky = r % WY, kx = r / WY;
-    const int gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
-    atomicAdd(reinterpret_cast<float4*>(mesh + ((int64_t)gx * ng + gy) * ng + gz), v);
+    if (any) {
+      const int gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
+      atomicAdd(reinterpret_cast<float4*>(mesh + ((int64_t)gx * ng + gy) * ng + gz), v);
+    }
+    kz += dKz; ky += dKy; kx += dKx;
+    if (kz >= WZ4) { kz -= WZ4; ky += 1; }
+    if (ky >= WY) { ky -= WY; kx += 1; }
   }
 }
 
@@ -289,40 +329,62 @@ readout_kernel(const float* __restrict__ m0, const float* __restrict__ m1,
 }
 
 __device__ __forceinline__ float wrap_box(float x, float ng, float inv_ng) {
-  x -= ng * floorf(x * inv_ng);
+  int unused;
+  x -= ng * fast_floor(x * inv_ng, unused);
   if (x >= ng) x -= ng;
   if (x < 0.f) x += ng;
   return x >= ng ? 0.f : x;
 }
 
 // One pass over the particles: gather the three force components at x (CIC),
-// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).
+// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).  The pass is latency-bound unless many
+// loads are in flight (profiles/r01_A: 15 warps stalled on the long scoreboard per issue), so a thread
+// first issues the 6 streaming loads of KB particles and only then starts the dependent gathers.
+// BRICK: a CTA of 256 threads walks half a brick (8 of its 16 y rows, all 8 x planes).
 template <bool BRICK>
-__global__ void __launch_bounds__(BRICK ? kBrickThreads : kThreads)
+__global__ void __launch_bounds__(kThreads, BRICK ? 3 : 4)
 readout_kick_drift_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
                           const float* __restrict__ fz, float* __restrict__ pos,
                           float* __restrict__ mom, int64_t n, int ngi, BrickMap bm, float kfac,
                           float dfac) {
   const float ng = (float)ngi, inv_ng = 1.f / ng;
   const float* const mesh[3] = {fx, fy, fz};
-  int qx0 = 0, qy0 = 0, qz0 = 0;
-  if (BRICK) bm.origin(blockIdx.x, qx0, qy0, qz0);
+  constexpr int KB = BRICK ? 4 : 1;
   constexpr int K = BRICK ? kPerThread : 1;
-#pragma unroll 2
-  for (int k = 0; k < K; ++k) {
-    int64_t p;
-    if (BRICK) p = bm.index(qx0, qy0, qz0, threadIdx.x + k * kBrickThreads);
-    else { p = (int64_t)blockIdx.x * kThreads + threadIdx.x; if (p >= n) return; }
-    const float x[3] = {ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p)};
-    const float m[3] = {ld_stream(mom + p), ld_stream(mom + n + p), ld_stream(mom + 2 * n + p)};
-    const Cic c = cic_of(x[0], x[1], x[2], ngi - 1);
-    float acc[3];
-    gather<3>(mesh, c, ngi, acc);
+  int64_t p0, plane = 0;
+  if (BRICK) {
+    int qx0, qy0, qz0;
+    bm.origin(blockIdx.x >> 1, qx0, qy0, qz0);
+    p0 = bm.index(qx0, qy0, qz0, threadIdx.x + kThreads * (blockIdx.x & 1));
+    plane = (int64_t)bm.np * bm.np;
+  } else {
+    p0 = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (p0 >= n) return;
+  }
+#pragma unroll 1
+  for (int k0 = 0; k0 < K; k0 += KB) {
+    float x[KB][3], m[KB][3];
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const float mn = fmaf(acc[d], kfac, m[d]);
-      __stcs(mom + d * n + p, mn);
-      __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[d]), ng, inv_ng));
+    for (int j = 0; j < KB; ++j) {
+      const int64_t p = p0 + (k0 + j) * plane;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        x[j][d] = ld_stream_rw(pos + d * n + p);
+        m[j][d] = ld_stream_rw(mom + d * n + p);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < KB; ++j) {
+      const int64_t p = p0 + (k0 + j) * plane;
+      const Cic c = cic_of(x[j][0], x[j][1], x[j][2], ngi - 1);
+      float acc[3];
+      gather<3>(mesh, c, ngi, acc);
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const float mn = fmaf(acc[d], kfac, m[j][d]);
+        __stcs(mom + d * n + p, mn);
+        __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[j][d]), ng, inv_ng));
+      }
     }
   }
 }
@@ -427,7 +489,7 @@ cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz
                                const ParticleOrder& ord, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   if (brick_ok(n, ord.np))
-    readout_kick_drift_kernel<true><<<(unsigned)(n / kBrick), kBrickThreads, 0, s>>>(
+    readout_kick_drift_kernel<true><<<(unsigned)(2 * (n / kBrick)), kThreads, 0, s>>>(
         fx, fy, fz, pos, mom, n, ng, brick_map(ord.np), kfac, dfac);
   else
     readout_kick_drift_kernel<false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng,
