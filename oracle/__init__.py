@@ -214,3 +214,36 @@ def readout_adjoint(mesh, pos, grad_out, grad_mesh=None):
     _load().orc_readout_adjoint(_p(mesh), _p(pos), ctypes.c_int64(n), ctypes.c_int(mesh.shape[0]),
                                 _p(go), _p(gm), _p(gpos))
     return gm, gpos
+
+
+def force_vjp(pos, ng, v, mode=KERNEL_PAPER, scale=1.0, mass=1.0):
+    """J_f(pos)^T v for f = force(pos) (R12); v, result [3][n]."""
+    pos, v = _f64(pos), _f64(v)
+    n = pos.shape[1]
+    gx = np.zeros((3, n))
+    _load().orc_force_vjp(_p(pos), ctypes.c_int64(n), ctypes.c_int(ng), ctypes.c_int(mode),
+                          ctypes.c_double(scale), ctypes.c_double(mass), _p(v), _p(gx))
+    return gx
+
+
+def nbody_vjp(traj, ng, np_side, omega_m, stages, gx, gp, mode=KERNEL_PAPER,
+              factor_mode=FACTORS_FASTPM):
+    """Reverse of nbody (R12): cotangents of the final (pos, mom) -> of the initial (pos, mom)."""
+    traj = _f64(traj)
+    gx, gp = _f64(gx).copy(), _f64(gp).copy()
+    n = traj.shape[2]
+    st = _f64(stages)
+    _load().orc_nbody_vjp(_p(traj), ctypes.c_int64(n), ctypes.c_int(ng), ctypes.c_int(np_side),
+                          ctypes.c_double(omega_m), ctypes.c_int(mode), ctypes.c_int(factor_mode),
+                          _p(st), ctypes.c_int(len(st) - 1), _p(gx), _p(gp))
+    return gx, gp
+
+
+def lpt_init_vjp(delta_lin, ng, omega_m, a0, order, gx, gp):
+    """Reverse of lpt_init (R12): cotangents of (pos, mom) -> of delta_lin [np^3]."""
+    d, gx, gp = _f64(delta_lin), _f64(gx), _f64(gp)
+    np_side = d.shape[0]
+    out = np.zeros(d.shape)
+    _load().orc_lpt_init_vjp(_p(d), ctypes.c_int(np_side), ctypes.c_int(ng), ctypes.c_double(omega_m),
+                             ctypes.c_double(a0), ctypes.c_int(order), _p(gx), _p(gp), _p(out))
+    return out

@@ -412,7 +412,7 @@ inline double kcomp(int64_t i, int64_t n, bool zero_nyquist) {
 // out = c2r( mult(k) * in ), mult = (i k_a)^[a>=0] (i k_b)^[b>=0] * (-1/k^2)^[inv_lap]
 // i k_d is zeroed at the Nyquist index of axis d; for a == b the product -(k_a)^2 keeps Nyquist.
 void spectral_apply(const std::vector<double>& in_k, int np, int a, int b, bool inv_lap,
-                    std::vector<double>& out_real) {
+                    std::vector<double>& out_real, bool conj_mult = false) {
   const int64_t n = np, nzh = np / 2 + 1;
   std::vector<double> tmp(in_k.size());
 #pragma omp parallel for schedule(static)
@@ -434,6 +434,7 @@ void spectral_apply(const std::vector<double>& in_k, int np, int a, int b, bool 
           for (int d = 0; d < 3; ++d) { const double k = kcomp(idx[d], n, false); k2 += k * k; }
           m *= (x == 0 && y == 0 && z == 0) ? 0.0 : -1.0 / k2;
         }
+        if (conj_mult) m = std::conj(m);   // transpose of a real convolution (R12)
         const cd v = m * cd(in_k[2 * i], in_k[2 * i + 1]);
         tmp[2 * i] = v.real();
         tmp[2 * i + 1] = v.imag();
@@ -515,6 +516,136 @@ void nbody_impl(double* pos, double* mom, int64_t n, int ng, int np, double om, 
     force_impl(pos, n, ng, mode, scale, mass, f.data(), nullptr);
     if (traj) std::memcpy(traj + (int64_t)(j + 1) * 3 * n, pos, sizeof(double) * 3 * n);
     kick_impl(mom, f.data(), n, kick_factor(om, ah, af, af, factor_mode));
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// R12  Reverse mode ("differentiable with respect to every component").
+// Every forward operation above is transposed in reverse order; nothing is merged or simplified.
+//   * T = c2r o mult(k) o r2c is a real periodic convolution; its transpose is the convolution
+//     whose multiplier is conj(mult) (correlation theorem).
+//   * paint^T (w.r.t. the mesh)  = readout ;  readout^T (w.r.t. the mesh) = paint with mass = cotangent;
+//     position derivatives by readout_grad_impl (R11).
+//   * wrap() has unit derivative.
+// ------------------------------------------------------------------------------------------
+
+// rho_bar = sum_d ForceGrids_d^T Fbar_d : r2c, multiply by conj(scale * i g_d / K^2), sum, c2r.
+void force_grids_transpose(double* const Fbar[3], int ng, int mode, double scale, double* rho_bar) {
+  const int64_t n = ng, nzh = ng / 2 + 1, nk = n * n * nzh;
+  std::vector<double> acc(2 * nk, 0.0), fk(2 * nk);
+  for (int d = 0; d < 3; ++d) {
+    r2c_impl(Fbar[d], ng, fk.data(), false);
+#pragma omp parallel for schedule(static)
+    for (int64_t x = 0; x < n; ++x)
+      for (int64_t y = 0; y < n; ++y)
+        for (int64_t z = 0; z < nzh; ++z) {
+          const int64_t idx[3] = {x, y, z};
+          double k2 = 0.0;
+          for (int e = 0; e < 3; ++e) k2 += lap_1d(mode, 2.0 * PI * freq_of(idx[e], n) / n);
+          const int f = freq_of(idx[d], n);
+          const bool zero = (x == 0 && y == 0 && z == 0);
+          const cd mult(0.0, scale * grad_1d(mode, 2.0 * PI * f / n, 2 * f == n) * (zero ? 0.0 : 1.0 / k2));
+          const int64_t i = (x * n + y) * nzh + z;
+          const cd v = std::conj(mult) * cd(fk[2 * i], fk[2 * i + 1]);
+          acc[2 * i] += v.real();
+          acc[2 * i + 1] += v.imag();
+        }
+  }
+  c2r_impl(acc.data(), ng, rho_bar, false);
+}
+
+// gx[3][n] += J_f(pos)^T v, where f = force_impl(pos) and v[3][n] is the cotangent of the force.
+void force_vjp_impl(const double* pos, int64_t n, int ng, int mode, double scale, double mass,
+                    const double* v, double* gx) {
+  const int64_t g3 = (int64_t)ng * ng * ng;
+  std::vector<double> rho(g3), F0(g3), F1(g3), F2(g3), B0(g3), B1(g3), B2(g3), rho_bar(g3), g(3 * n);
+  paint_impl(pos, nullptr, mass, n, ng, rho.data());
+  double* F[3] = {F0.data(), F1.data(), F2.data()};
+  force_grids_impl(rho.data(), ng, mode, scale, F);
+  double* Fbar[3] = {B0.data(), B1.data(), B2.data()};
+  for (int d = 0; d < 3; ++d) {
+    // f_d = readout(F_d, pos):  cotangent of the mesh = paint(pos, mass = v_d);
+    //                           cotangent of pos     = v_d * sum_c F_d[c] dW/dx
+    paint_impl(pos, v + d * n, 0.0, n, ng, Fbar[d]);
+    readout_grad_impl(F[d], pos, n, ng, g.data());
+    for (int e = 0; e < 3; ++e)
+      for (int64_t p = 0; p < n; ++p) gx[e * n + p] += v[d * n + p] * g[e * n + p];
+  }
+  force_grids_transpose(Fbar, ng, mode, scale, rho_bar.data());
+  // rho = paint(pos, mass): cotangent of pos = mass * sum_c rho_bar[c] dW/dx
+  readout_grad_impl(rho_bar.data(), pos, n, ng, g.data());
+  for (int64_t i = 0; i < 3 * n; ++i) gx[i] += mass * g[i];
+}
+
+// Reverse of nbody_impl.  traj[(n_steps+1)][3][n]: positions at every force evaluation.
+// In: gx, gp = dL/d(final pos, final mom).  Out: gx, gp = dL/d(initial pos, initial mom).
+void nbody_vjp_impl(const double* traj, int64_t n, int ng, int np, double om, int mode,
+                    int factor_mode, const double* stages, int n_steps, double* gx, double* gp) {
+  const double B = (double)ng / np, mass = B * B * B, scale = 1.5 * om;
+  std::vector<double> v(3 * n);
+  for (int j = n_steps - 1; j >= 0; --j) {
+    const double ai = stages[j], af = stages[j + 1], ah = std::sqrt(ai * af);
+    const double k1 = kick_factor(om, ai, ai, ah, factor_mode);
+    const double dr = drift_factor(om, ai, ah, af, factor_mode);
+    const double k2 = kick_factor(om, ah, af, af, factor_mode);
+    const double* x1 = traj + (int64_t)(j + 1) * 3 * n;
+    const double* x0 = traj + (int64_t)j * 3 * n;
+    // mom += k2 f(x_{j+1})
+    for (int64_t i = 0; i < 3 * n; ++i) v[i] = k2 * gp[i];
+    force_vjp_impl(x1, n, ng, mode, scale, mass, v.data(), gx);
+    // pos = wrap(pos + dr mom)
+    for (int64_t i = 0; i < 3 * n; ++i) gp[i] += dr * gx[i];
+    // mom += k1 f(x_j)
+    for (int64_t i = 0; i < 3 * n; ++i) v[i] = k1 * gp[i];
+    force_vjp_impl(x0, n, ng, mode, scale, mass, v.data(), gx);
+  }
+}
+
+// Reverse of lpt_init_impl: gdelta[np^3] = dL/d(delta_lin) given gx, gp = dL/d(pos, mom).
+void lpt_init_vjp_impl(const double* delta_lin, int np, int ng, double om, double a0, int order,
+                       const double* gx, const double* gp, double* gdelta) {
+  const int64_t n3 = (int64_t)np * np * np, nk = (int64_t)np * np * (np / 2 + 1);
+  const int B = ng / np;
+  const Growth g = growth_at(om, a0);
+  const double pre = a0 * a0 * g.E;
+  std::vector<double> tmp, rk(2 * nk), bar(n3);
+  for (int64_t i = 0; i < n3; ++i) gdelta[i] = 0.0;
+  // pos = q B + (D1 psi1 + D2 psi2) B ; mom = pre (f1 D1 psi1 + f2 D2 psi2) B
+  // psi1_d = T[(i k_d)(-1/k^2)] (-delta)
+  for (int d = 0; d < 3; ++d) {
+    for (int64_t i = 0; i < n3; ++i)
+      bar[i] = B * (g.D1 * gx[d * n3 + i] + pre * g.f1 * g.D1 * gp[d * n3 + i]);
+    r2c_impl(bar.data(), np, rk.data(), false);
+    spectral_apply(rk, np, d, -1, true, tmp, true);
+    for (int64_t i = 0; i < n3; ++i) gdelta[i] -= tmp[i];
+  }
+  if (order < 2) return;
+  // psi2_d = T[(i k_d)(-1/k^2)] S
+  std::vector<double> Sbar(n3, 0.0);
+  for (int d = 0; d < 3; ++d) {
+    for (int64_t i = 0; i < n3; ++i)
+      bar[i] = B * (g.D2 * gx[d * n3 + i] + pre * g.f2 * g.D2 * gp[d * n3 + i]);
+    r2c_impl(bar.data(), np, rk.data(), false);
+    spectral_apply(rk, np, d, -1, true, tmp, true);
+    for (int64_t i = 0; i < n3; ++i) Sbar[i] += tmp[i];
+  }
+  // S = pxx pyy + pxx pzz + pyy pzz - pxy^2 - pxz^2 - pyz^2 ,  p_ij = T[(i k_i)(i k_j)(-1/k^2)] delta
+  std::vector<double> dk(2 * nk), phi[6];
+  r2c_impl(delta_lin, np, dk.data(), false);
+  const int ia[6] = {0, 1, 2, 0, 0, 1}, ib[6] = {0, 1, 2, 1, 2, 2};
+  for (int c = 0; c < 6; ++c) spectral_apply(dk, np, ia[c], ib[c], true, phi[c]);
+  for (int c = 0; c < 6; ++c) {
+    for (int64_t i = 0; i < n3; ++i) {
+      double dS;
+      if (c == 0) dS = phi[1][i] + phi[2][i];
+      else if (c == 1) dS = phi[0][i] + phi[2][i];
+      else if (c == 2) dS = phi[0][i] + phi[1][i];
+      else dS = -2.0 * phi[c][i];
+      bar[i] = Sbar[i] * dS;
+    }
+    r2c_impl(bar.data(), np, rk.data(), false);
+    spectral_apply(rk, np, ia[c], ib[c], true, tmp, true);
+    for (int64_t i = 0; i < n3; ++i) gdelta[i] += tmp[i];
   }
 }
 
@@ -664,6 +795,21 @@ void orc_readout_adjoint(const double* mesh, const double* pos, int64_t n, int n
     for (int d = 0; d < 3; ++d)
       for (int64_t p = 0; p < n; ++p) grad_pos[d * n + p] *= grad_out[p];
   }
+}
+
+
+// ---- R12 reverse mode ---------------------------------------------------------------------------
+void orc_force_vjp(const double* pos, int64_t n, int ng, int mode, double scale, double mass,
+                   const double* v, double* gx) {
+  force_vjp_impl(pos, n, ng, mode, scale, mass, v, gx);
+}
+void orc_nbody_vjp(const double* traj, int64_t n, int ng, int np, double om, int mode, int factor_mode,
+                   const double* stages, int n_steps, double* gx, double* gp) {
+  nbody_vjp_impl(traj, n, ng, np, om, mode, factor_mode, stages, n_steps, gx, gp);
+}
+void orc_lpt_init_vjp(const double* delta_lin, int np, int ng, double om, double a0, int order,
+                      const double* gx, const double* gp, double* gdelta) {
+  lpt_init_vjp_impl(delta_lin, np, ng, om, a0, order, gx, gp, gdelta);
 }
 
 }  // extern "C"
