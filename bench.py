@@ -50,6 +50,7 @@ def algorithmic_bytes(n_p, ng):
         "fft_cols_y": 16 * n_k,
         "fft_cols_x": 16 * n_k,
         "fft_z_c2r": 8 * n_k + 4 * n_g,
+        "fft_z_c2r3": 24 * n_k + 12 * n_g,      # fused path: 3 components, interleaved output (pad not credited)
         "apply_force_kernel": 32 * n_k,
         "fft_x_force": 24 * n_k,
         "fft_y_inv3": 40 * n_k,
@@ -78,7 +79,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "25"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -174,7 +175,7 @@ def workload_name(cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=37)   # + 3 warm-up = C4's 40-step schedule
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=sorted(fi.CONFIGS))

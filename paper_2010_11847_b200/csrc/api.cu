@@ -89,14 +89,16 @@ inline float particle_mass(const fpm_ctx* ctx) {
 }
 
 // paint -> r2c -> transfer function -> 3x c2r : the three force meshes of Alg. 3 ForceGrids(local)
-int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n) {
+// interleaved: (fused path only) the components go to one float4-per-cell mesh that overlays
+// rho | F[0] | F[1] | F[2] (16 ng^3 contiguous bytes; rho is dead once the z r2c pass has read it).
+int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, bool interleaved = false) {
   const int ng = ctx->cfg.ng;
   cudaStream_t s = ctx->stream;
   Profiler* pr = &ctx->prof;
   { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s)); }
   if (ctx->cfg.force_path == FPM_FORCE_FUSED) {
     FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F,
-                                  (float)(1.5 * ctx->cfg.omega_m), s, pr));
+                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr));
     return FPM_OK;
   }
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
@@ -112,11 +114,16 @@ int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n) 
 // One PM step: force at the current positions, p += f K, x = wrap(x + p D).
 int pm_step(fpm_ctx* ctx, const Workspace& w, float* pos, float* mom, int64_t n, double kfac,
             double dfac) {
-  const int rc = force_meshes(ctx, w, pos, n);
+  const bool f4 = ctx->cfg.force_path == FPM_FORCE_FUSED;
+  const int rc = force_meshes(ctx, w, pos, n, f4);
   if (rc != FPM_OK) return rc;
   ProfScope sc(&ctx->prof, K_READOUT_KICK_DRIFT);
-  FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
-                                   (float)dfac, order_of(ctx, n), ctx->stream));
+  if (f4)
+    FPM_CUDA(ctx, readout_kick_drift(w.rho, nullptr, nullptr, pos, mom, n, ctx->cfg.ng, (float)kfac,
+                                     (float)dfac, order_of(ctx, n), ctx->stream));
+  else
+    FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
+                                     (float)dfac, order_of(ctx, n), ctx->stream));
   return FPM_OK;
 }
 

@@ -129,7 +129,7 @@ cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t
 // third).  wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.
 template <int N>
 cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
-                             float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
                              cudaStream_t s, Profiler* prof) {
   constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>(), T = col_tile<N>();
   const int64_t nrows = (int64_t)N * N;
@@ -173,6 +173,17 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     kern<<<grid, threads, smem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * nzh, nzh, nzh, t.stage_n, kt.grad);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+  }
+  if (F4) {   // interleaved (F_x, F_y, F_z, -) per cell for the fused readout
+    ProfScope sc(prof, K_FFT_Z_C2R3);
+    constexpr int zthreads = G * Plan<M>::P;
+    const size_t zsmem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
+    auto kern = fft_z_c2r3_kernel<N>;
+    e = set_smem(kern, zsmem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((nrows + G - 1) / G), zthreads, zsmem, s>>>(wb, dk, wc, F4, nrows, t.stage_m, t.full,
+                                                                (float)(1.0 / ((double)N * N * N)), kt.grad);
+    return cudaGetLastError();
   }
   e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof);
   if (e != cudaSuccess) return e;
@@ -235,10 +246,10 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
 }
 
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
-                            float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                            float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
                             cudaStream_t s, Profiler* prof) {
   if (kt.n != t.n) return cudaErrorInvalidValue;
-  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, scale, s, prof)
+  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof)
 }
 
 }  // namespace fpm

@@ -225,4 +225,64 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
   for (int e = 0; e < E; ++e) dst[p + P * e] = make_float2(v[e].y * scale, v[e].x * scale);
 }
 
+// The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved
+// per cell as float4 (F_x, F_y, F_z, unused): the readout then needs one 16-byte gather per CIC
+// corner instead of three 4-byte ones (profiles/r01_B: the gather was request- and latency-bound).
+// A block inverts its G rows for component 0, 1, 2 in turn; the three 4-byte stores that make up a
+// cell's sector are issued within microseconds of each other and merge in L2 before write-back.
+// g(w_z) of Eq. 5 is applied on load to component 2 (see fft_z_c2r_kernel).
+template <int N>
+__global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
+fft_z_c2r3_kernel(const float2* __restrict__ in0, const float2* __restrict__ in1,
+                  const float2* __restrict__ in2, float* __restrict__ out4, int64_t nrows,
+                  const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
+                  const float* __restrict__ gz) {
+  extern __shared__ float2 smem[];
+  constexpr int M = N / 2;
+  using PL = Plan<M>;
+  constexpr int E = PL::E, P = PL::P, G = z_rows<N>();
+  const int p = threadIdx.x % P, g = threadIdx.x / P;
+  const int64_t row = (int64_t)blockIdx.x * G + g;
+  const bool ok = row < nrows;
+  RowSmem sm{smem + g * row_pitch(M)};
+#pragma unroll 1
+  for (int comp = 0; comp < 3; ++comp) {
+    const float2* src = (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * (M + 1);
+    float2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int k = p + P * e;
+      float2 z = make_float2(0.f, 0.f);
+      if (ok) {
+        float2 xk = src[k], xm = src[M - k];
+        if (comp == 2) {
+          const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
+          xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
+        }
+        if (k == 0) {
+          z = make_float2(xk.x + xm.x, xk.x - xm.x);
+        } else {
+          const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
+          const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
+          const float2 w = __ldg(twn + k);
+          const float2 b = cmul(d, make_float2(w.x, -w.y));
+          z = make_float2(a.x - b.y, a.y + b.x);
+        }
+      }
+      v[e] = cswap(z);
+    }
+    fft_line<M>(v, p, sm, tw);
+    if (ok) {
+      float* dst = out4 + row * (4 * (int64_t)N) + comp;
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const int z = 2 * (p + P * e);
+        dst[4 * z] = v[e].y * scale;
+        dst[4 * z + 4] = v[e].x * scale;
+      }
+    }
+    if constexpr (PL::NST > 1) __syncthreads();   // the exchange buffer is reused by the next component
+  }
+}
+
 }  // namespace fpm

@@ -13,7 +13,7 @@ namespace fpm {
 // ---- per-kernel accounting: launch counter (always) + CUDA-event timing (when enabled) --------
 enum KernelId {
   K_PAINT = 0, K_FFT_Z_R2C, K_FFT_Y, K_FFT_X, K_FFT_Z_C2R, K_GREEN, K_READOUT, K_READOUT_KICK_DRIFT,
-  K_KICK, K_DRIFT, K_READOUT_GRAD, K_LPT, K_FFT_X_FORCE, K_FFT_Y_INV3, K_MEMSET, K_COUNT
+  K_KICK, K_DRIFT, K_READOUT_GRAD, K_LPT, K_FFT_X_FORCE, K_FFT_Y_INV3, K_MEMSET, K_FFT_Z_C2R3, K_COUNT
 };
 const char* kernel_name(int kid);
 
@@ -74,9 +74,10 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
                     Profiler* prof = nullptr);
 
 // paint'ed density -> the three force meshes F[0..2] with the transfer function fused into the
-// transform passes (fft.cu); scale = 1.5 omega_m (or 1)
+// transform passes (fft.cu); scale = 1.5 omega_m (or 1).  F4 != nullptr: the three components are
+// written interleaved per cell as float4 (x, y, z, unused) into F4[4 ng^3] instead of F[0..2].
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
-                            float2* wa, float2* wb, float2* wc, float* const* F, float scale,
+                            float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
                             cudaStream_t s, Profiler* prof = nullptr);
 
 // ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
@@ -100,6 +101,7 @@ cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale
 cudaError_t kick(float* mom, const float* force, int64_t n3, float fac, cudaStream_t s);
 cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, cudaStream_t s);
 // mom += force(pos) * kfac ; pos = wrap(pos + mom * dfac), gathering the three force meshes
+// fy == fz == nullptr: fx is the interleaved float4 force mesh of fft_force_fused
 cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
                                float* mom, int64_t n, int ng, float kfac, float dfac,
                                const ParticleOrder& ord, cudaStream_t s);

@@ -254,7 +254,6 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   constexpr int WZ4 = WZ / 4;
   // (kx, ky, kz) of group gidx advance incrementally: no division in the loop
   constexpr int dKz = kBrickThreads % WZ4, dRow = kBrickThreads / WZ4, dKy = dRow % WY, dKx = dRow / WY;
-  static_assert(kThreads * 2 == kBrickThreads && BX == kPerThread, "half-brick walk of readout_kick_drift");
   static_assert(dKy + 1 < WY, "one carry per step");
   int kz = tid % WZ4, ky = (tid / WZ4) % WY, kx = (tid / WZ4) / WY;
   for (int gidx = tid; gidx < kWinCells / 4; gidx += kBrickThreads) {
@@ -279,26 +278,54 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
 }
 
 // ---- readout -----------------------------------------------------------------------------------
+// 32-bit cell indices (ng <= 1024: ng^3 <= 2^30), so every gather address is one IMAD.WIDE.U32; the
+// 64-bit row arithmetic was most of the instruction count of the readout kernels (profiles/r01_B).
 template <int NMESH>
-__device__ __forceinline__ void gather(const float* const* mesh, const Cic& c, int64_t g,
+__device__ __forceinline__ void gather(const float* const* mesh, const Cic& c, unsigned g,
                                        float (&acc)[NMESH]) {
   const float wx[2] = {1.f - c.t[0], c.t[0]};
   const float wy[2] = {1.f - c.t[1], c.t[1]};
   const float wz[2] = {1.f - c.t[2], c.t[2]};
-  const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]};
+  const unsigned ix[2] = {(unsigned)c.i0[0] * g, (unsigned)c.i1[0] * g};
+  const unsigned iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]};
+  const unsigned z0 = (unsigned)c.i0[2], z1 = (unsigned)c.i1[2];
 #pragma unroll
   for (int k = 0; k < NMESH; ++k) acc[k] = 0.f;
 #pragma unroll
   for (int a = 0; a < 2; ++a)
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
-      const int64_t row = ((int64_t)ix[a] * g + iy[b]) * g;
+      const unsigned row = (ix[a] + iy[b]) * g;
       const float w = wx[a] * wy[b];
+      const float w0 = w * wz[0], w1 = w * wz[1];
 #pragma unroll
       for (int k = 0; k < NMESH; ++k) {
-        acc[k] = fmaf(__ldg(mesh[k] + row + c.i0[2]), w * wz[0], acc[k]);
-        acc[k] = fmaf(__ldg(mesh[k] + row + c.i1[2]), w * wz[1], acc[k]);
+        acc[k] = fmaf(__ldg(mesh[k] + (row + z0)), w0, acc[k]);
+        acc[k] = fmaf(__ldg(mesh[k] + (row + z1)), w1, acc[k]);
       }
+    }
+}
+
+// The three force components interleaved per cell (x, y, z, unused): one 16-byte load per corner.
+__device__ __forceinline__ void gather4(const float4* __restrict__ mesh, const Cic& c, unsigned g,
+                                        float (&acc)[3]) {
+  const float wx[2] = {1.f - c.t[0], c.t[0]};
+  const float wy[2] = {1.f - c.t[1], c.t[1]};
+  const float wz[2] = {1.f - c.t[2], c.t[2]};
+  const unsigned ix[2] = {(unsigned)c.i0[0] * g, (unsigned)c.i1[0] * g};
+  const unsigned iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]};
+  const unsigned z0 = (unsigned)c.i0[2], z1 = (unsigned)c.i1[2];
+  acc[0] = acc[1] = acc[2] = 0.f;
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const unsigned row = (ix[a] + iy[b]) * g;
+      const float w = wx[a] * wy[b];
+      const float w0 = w * wz[0], w1 = w * wz[1];
+      const float4 v0 = __ldg(mesh + (row + z0)), v1 = __ldg(mesh + (row + z1));
+      acc[0] = fmaf(v0.x, w0, acc[0]); acc[1] = fmaf(v0.y, w0, acc[1]); acc[2] = fmaf(v0.z, w0, acc[2]);
+      acc[0] = fmaf(v1.x, w1, acc[0]); acc[1] = fmaf(v1.y, w1, acc[1]); acc[2] = fmaf(v1.z, w1, acc[2]);
     }
 }
 
@@ -337,55 +364,109 @@ __device__ __forceinline__ float wrap_box(float x, float ng, float inv_ng) {
 }
 
 // One pass over the particles: gather the three force components at x (CIC),
-// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).  The pass is latency-bound unless many
-// loads are in flight (profiles/r01_A: 15 warps stalled on the long scoreboard per issue), so a thread
-// first issues the 6 streaming loads of KB particles and only then starts the dependent gathers.
-// BRICK: a CTA of 256 threads walks half a brick (8 of its 16 y rows, all 8 x planes).
-template <bool BRICK>
-__global__ void __launch_bounds__(kThreads, BRICK ? 3 : 4)
+// p += f * kfac (Eq. 2), x = wrap(x + p * dfac) (Eq. 1).  Generic variant: one thread per particle in
+// memory order, for particle sets that are not a full lattice (the brick variant follows).
+// F4: fx is the interleaved (F_x, F_y, F_z, -) mesh written by fft_z_c2r3_kernel.
+template <bool F4>
+__global__ void __launch_bounds__(kThreads, 4)
 readout_kick_drift_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
                           const float* __restrict__ fz, float* __restrict__ pos,
-                          float* __restrict__ mom, int64_t n, int ngi, BrickMap bm, float kfac,
-                          float dfac) {
+                          float* __restrict__ mom, int64_t n, int ngi, float kfac, float dfac) {
   const float ng = (float)ngi, inv_ng = 1.f / ng;
   const float* const mesh[3] = {fx, fy, fz};
-  constexpr int KB = BRICK ? 4 : 1;
-  constexpr int K = BRICK ? kPerThread : 1;
-  int64_t p0, plane = 0;
-  if (BRICK) {
-    int qx0, qy0, qz0;
-    bm.origin(blockIdx.x >> 1, qx0, qy0, qz0);
-    p0 = bm.index(qx0, qy0, qz0, threadIdx.x + kThreads * (blockIdx.x & 1));
-    plane = (int64_t)bm.np * bm.np;
-  } else {
-    p0 = (int64_t)blockIdx.x * kThreads + threadIdx.x;
-    if (p0 >= n) return;
+  const int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  if (p >= n) return;
+  float x[3], m[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    x[d] = ld_stream_rw(pos + d * n + p);
+    m[d] = ld_stream_rw(mom + d * n + p);
   }
+  const Cic c = cic_of(x[0], x[1], x[2], ngi - 1);
+  float acc[3];
+  if (F4) gather4(reinterpret_cast<const float4*>(fx), c, ngi, acc);
+  else gather<3>(mesh, c, ngi, acc);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const float mn = fmaf(acc[d], kfac, m[d]);
+    __stcs(mom + d * n + p, mn);
+    __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[d]), ng, inv_ng));
+  }
+}
+
+// ---- pipelined brick variant ----------------------------------------------------------------
+// The streaming operands (x, p of the next planes) are fetched with cp.async into a small
+// shared-memory ring while the current planes are gathered, so the DRAM latency of the 48 B/particle
+// stream is never on a warp's critical path.  Each warp copies exactly the 32 particles it will
+// process (12 runs of 128 B per batch = 96 16-byte copies, 3 per lane), so the ring needs only
+// warp-level synchronisation.  .cg copies bypass L1, which stays reserved for the mesh gathers.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <int STAGES, int KB, int MINB, bool F4 = false>
+__global__ void __launch_bounds__(kThreads, MINB)
+rkd_pipelined_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
+                     const float* __restrict__ fz, float* __restrict__ pos, float* __restrict__ mom,
+                     int64_t n, int ngi, BrickMap bm, float kfac, float dfac) {
+  static_assert(BX % KB == 0, "batch shape");
+  constexpr int NB = BX / KB;             // batches (groups of KB x-planes) per half-brick
+  constexpr int DIST = STAGES - 1;        // prefetch distance
+  constexpr int NCP = KB * 6 * 8;         // 16-byte copies per warp and batch
+  constexpr int CPL = (NCP + 31) / 32;
+  __shared__ __align__(16) float ring[STAGES][KB][6][kThreads];
+  const float ng = (float)ngi, inv_ng = 1.f / ng;
+  const float* const mesh[3] = {fx, fy, fz};
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  int qx0, qy0, qz0;
+  static_assert(kThreads == (BY / 2) * BZ, "a CTA walks half a brick: 8 of its 16 y rows, all x planes");
+  bm.origin(blockIdx.x >> 1, qx0, qy0, qz0);
+  const int64_t plane = (int64_t)bm.np * bm.np;
+  // lattice row of this warp in plane 0 of the brick: lane 0's particle index
+  const int64_t row0 = ((int64_t)qx0 * bm.np + (qy0 + (BY / 2) * (blockIdx.x & 1) + warp)) * bm.np + qz0;
+
+  auto issue = [&](int batch) {
+    const int st = batch % STAGES;
+#pragma unroll
+    for (int i = 0; i < CPL; ++i) {
+      const int t = lane + 32 * i, r = t >> 3, c = t & 7;
+      if (NCP % 32 != 0 && t >= NCP) break;
+      const int j = r / 6, a = r - 6 * j;
+      const float* src = (a < 3 ? pos + a * n : mom + (a - 3) * n) + row0 + (int64_t)(batch * KB + j) * plane + 4 * c;
+      cp_async16(&ring[st][j][a][warp * 32 + 4 * c], src);
+    }
+  };
+#pragma unroll
+  for (int b = 0; b < DIST; ++b) { if (b < NB) issue(b); cp_async_commit(); }
 #pragma unroll 1
-  for (int k0 = 0; k0 < K; k0 += KB) {
-    float x[KB][3], m[KB][3];
+  for (int b = 0; b < NB; ++b) {
+    if (b + DIST < NB) issue(b + DIST);
+    cp_async_commit();
+    cp_async_wait<DIST>();
+    __syncwarp();
+    const int st = b % STAGES;
 #pragma unroll
     for (int j = 0; j < KB; ++j) {
-      const int64_t p = p0 + (k0 + j) * plane;
+      const int64_t p = row0 + lane + (int64_t)(b * KB + j) * plane;
+      float x[3], m[3];
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        x[j][d] = ld_stream_rw(pos + d * n + p);
-        m[j][d] = ld_stream_rw(mom + d * n + p);
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < KB; ++j) {
-      const int64_t p = p0 + (k0 + j) * plane;
-      const Cic c = cic_of(x[j][0], x[j][1], x[j][2], ngi - 1);
+      for (int d = 0; d < 3; ++d) { x[d] = ring[st][j][d][tid]; m[d] = ring[st][j][3 + d][tid]; }
+      const Cic c = cic_of(x[0], x[1], x[2], ngi - 1);
       float acc[3];
-      gather<3>(mesh, c, ngi, acc);
+      if (F4) gather4(reinterpret_cast<const float4*>(fx), c, ngi, acc);
+      else gather<3>(mesh, c, ngi, acc);
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const float mn = fmaf(acc[d], kfac, m[j][d]);
+        const float mn = fmaf(acc[d], kfac, m[d]);
         __stcs(mom + d * n + p, mn);
-        __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[j][d]), ng, inv_ng));
+        __stcs(pos + d * n + p, wrap_box(fmaf(mn, dfac, x[d]), ng, inv_ng));
       }
     }
+    __syncwarp();   // the stage is refilled by the issue of the next iteration
   }
 }
 
@@ -488,12 +569,21 @@ cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz
                                float* mom, int64_t n, int ng, float kfac, float dfac,
                                const ParticleOrder& ord, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  if (brick_ok(n, ord.np))
-    readout_kick_drift_kernel<true><<<(unsigned)(2 * (n / kBrick)), kThreads, 0, s>>>(
-        fx, fy, fz, pos, mom, n, ng, brick_map(ord.np), kfac, dfac);
+  const bool f4 = (fy == nullptr);   // interleaved force mesh
+  const bool aligned = ((reinterpret_cast<uintptr_t>(pos) | reinterpret_cast<uintptr_t>(mom)) & 15) == 0;
+  if (brick_ok(n, ord.np) && aligned) {
+    const unsigned grid = (unsigned)(2 * (n / kBrick));
+    const BrickMap bm = brick_map(ord.np);
+    if (f4)
+      rkd_pipelined_kernel<3, 1, 4, true><<<grid, kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, bm, kfac, dfac);
+    else
+      rkd_pipelined_kernel<3, 1, 4, false><<<grid, kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, bm, kfac, dfac);
+    return cudaGetLastError();
+  }
+  if (f4)
+    readout_kick_drift_kernel<true><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, kfac, dfac);
   else
-    readout_kick_drift_kernel<false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng,
-                                                                       BrickMap{0, 1, 1}, kfac, dfac);
+    readout_kick_drift_kernel<false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, kfac, dfac);
   return cudaGetLastError();
 }
 

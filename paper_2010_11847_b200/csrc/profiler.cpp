@@ -8,7 +8,7 @@ const char* kernel_name(int kid) {
   static const char* names[K_COUNT] = {
       "paint", "fft_z_r2c", "fft_cols_y", "fft_cols_x", "fft_z_c2r", "apply_force_kernel", "readout",
       "readout_kick_drift", "kick", "drift", "readout_grad", "lpt_elementwise", "fft_x_force",
-      "fft_y_inv3", "memset"};
+      "fft_y_inv3", "memset", "fft_z_c2r3"};
   return (kid >= 0 && kid < K_COUNT) ? names[kid] : "?";
 }
 

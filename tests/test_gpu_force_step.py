@@ -115,9 +115,9 @@ def test_lpt_init_with_resolution_factor_two(fpm, oracle):
     assert rel_l2(host(mom), rmom) < 1e-5
 
 
-def _run_config(fpm, oracle, cfg, order):
+def _run_config(fpm, oracle, cfg, order, force_path=0):
     delta = fi.linear_field(cfg.np_side, cfg.box, cfg.seed)
-    ctx = fpm.FPM(cfg.ng, cfg.np_side, box=cfg.box)
+    ctx = fpm.FPM(cfg.ng, cfg.np_side, box=cfg.box, force_path=force_path)
     pos, mom = ctx.lpt_init(dev(delta), cfg.a0, order)
     # the oracle starts from the SAME fp32 initial state, widened
     p0, m0 = host(pos).astype(np.float64), host(mom).astype(np.float64)
@@ -127,9 +127,10 @@ def _run_config(fpm, oracle, cfg, order):
     return ctx, host(pos), host(mom), rpos, rmom
 
 
-def test_full_run_C1_matches_oracle(fpm, oracle):
+@pytest.mark.parametrize("force_path", [0, 1])
+def test_full_run_C1_matches_oracle(fpm, oracle, force_path):
     cfg = fi.CONFIGS["C1"]
-    ctx, pos, mom, rpos, rmom = _run_config(fpm, oracle, cfg, cfg.lpt_order)
+    ctx, pos, mom, rpos, rmom = _run_config(fpm, oracle, cfg, cfg.lpt_order, force_path)
     dist = periodic_dist(pos, rpos, cfg.ng)
     assert dist.max() < 1e-3, f"max {dist.max():.2e} rms {np.sqrt((dist**2).mean()):.2e}"
     assert rel_l2(mom, rmom) < 1e-4
@@ -137,3 +138,30 @@ def test_full_run_C1_matches_oracle(fpm, oracle):
     k, pk_ref, nm = oracle.power(oracle.paint(rpos, cfg.ng, mass_const=b3), cfg.box)
     _, pk_got, _ = oracle.power(oracle.paint(pos.astype(np.float64), cfg.ng, mass_const=b3), cfg.box)
     assert np.max(np.abs(pk_got / pk_ref - 1)) < 1e-4
+
+
+@pytest.mark.parametrize("np_side,ng", [(64, 64), (32, 64)])
+def test_short_run_fused_path_spanning_several_bricks(fpm, oracle, np_side, ng):
+    """4 FastPM steps through the fused path (interleaved force mesh, pipelined brick readout)."""
+    cfg = fi.Config("T", np_side, ng, 100.0, 2, 4)
+    ctx, pos, mom, rpos, rmom = _run_config(fpm, oracle, cfg, 2, force_path=1)
+    dist = periodic_dist(pos, rpos, cfg.ng)
+    assert dist.max() < 1e-3, f"max {dist.max():.2e}"
+    assert rel_l2(mom, rmom) < 1e-4
+
+
+@pytest.mark.parametrize("force_path", [0, 1])
+def test_pm_step_with_arbitrary_particle_count(fpm, oracle, force_path):
+    """n is not a lattice set: the generic (non-brick) kernels run; one PM step against the oracle."""
+    ng, n = 32, 5003
+    pos = fi.random_particles(n, ng, 17, clustered=True)
+    mom = (0.1 * np.random.default_rng(3).standard_normal((3, n))).astype(np.float32)
+    ctx = fpm.FPM(ng, ng, force_path=force_path)
+    kf, dr = ctx.kick_factor(0.2, 0.2, 0.3), ctx.drift_factor(0.2, 0.25, 0.3)
+    dpos, dmom = dev(pos), dev(mom)
+    ctx.pm_step(dpos, dmom, kf, dr)
+    f = oracle.force(pos.astype(np.float64), ng, scale=1.5 * OM, mass=1.0)
+    rmom = oracle.kick(mom.astype(np.float64), f, kf)
+    rpos = oracle.drift(pos.astype(np.float64), rmom, dr, ng)
+    assert rel_l2(host(dmom), rmom) < 1e-5
+    assert periodic_dist(host(dpos), rpos, ng).max() < 1e-4
