@@ -176,13 +176,14 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   if (F4) {   // interleaved (F_x, F_y, F_z, -) per cell for the fused readout
     ProfScope sc(prof, K_FFT_Z_C2R3);
-    constexpr int zthreads = G * Plan<M>::P;
-    const size_t zsmem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
+    constexpr int GC = z3_rows<N>();
+    const size_t zsmem = z3_smem_bytes<N>();
     auto kern = fft_z_c2r3_kernel<N>;
     e = set_smem(kern, zsmem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((nrows + G - 1) / G), zthreads, zsmem, s>>>(wb, dk, wc, F4, nrows, t.stage_m, t.full,
-                                                                (float)(1.0 / ((double)N * N * N)), kt.grad);
+    kern<<<(unsigned)((nrows + GC - 1) / GC), z3_threads<N>(), zsmem, s>>>(
+        wb, dk, wc, reinterpret_cast<float4*>(F4), nrows, t.stage_m, t.full,
+        (float)(1.0 / ((double)N * N * N)), kt.grad);
     return cudaGetLastError();
   }
   e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof);

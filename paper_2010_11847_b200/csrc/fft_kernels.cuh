@@ -226,63 +226,75 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
 }
 
 // The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved
-// per cell as float4 (F_x, F_y, F_z, unused): the readout then needs one 16-byte gather per CIC
-// corner instead of three 4-byte ones (profiles/r01_B: the gather was request- and latency-bound).
-// A block inverts its G rows for component 0, 1, 2 in turn; the three 4-byte stores that make up a
-// cell's sector are issued within microseconds of each other and merge in L2 before write-back.
+// per cell as float4 (F_x, F_y, F_z, 0): the readout then needs one 16-byte gather per CIC corner
+// instead of three 4-byte ones (profiles/r01_B: the gather was request- and latency-bound).
+// A block owns GC rows; its three thread groups (GC*P threads each, whole warps) invert the rows of
+// component 0, 1, 2 concurrently, each with its own exchange buffer, park the real rows there, and
+// the block then writes its GC*N cells as fully coalesced float4.
 // g(w_z) of Eq. 5 is applied on load to component 2 (see fft_z_c2r_kernel).
+template <int N> __host__ __device__ constexpr int z3_rows() {
+  constexpr int g = z_rows<N>() / 4;
+  return g < 1 ? 1 : g;
+}
+template <int N> __host__ __device__ constexpr int z3_threads() { return 3 * z3_rows<N>() * Plan<N / 2>::P; }
+template <int N> __host__ __device__ constexpr size_t z3_smem_bytes() {
+  return sizeof(float2) * 3 * (size_t)z3_rows<N>() * row_pitch(N / 2);
+}
+
 template <int N>
-__global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
+__global__ void __launch_bounds__(z3_threads<N>())
 fft_z_c2r3_kernel(const float2* __restrict__ in0, const float2* __restrict__ in1,
-                  const float2* __restrict__ in2, float* __restrict__ out4, int64_t nrows,
+                  const float2* __restrict__ in2, float4* __restrict__ out4, int64_t nrows,
                   const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
                   const float* __restrict__ gz) {
   extern __shared__ float2 smem[];
   constexpr int M = N / 2;
   using PL = Plan<M>;
-  constexpr int E = PL::E, P = PL::P, G = z_rows<N>();
-  const int p = threadIdx.x % P, g = threadIdx.x / P;
-  const int64_t row = (int64_t)blockIdx.x * G + g;
+  constexpr int E = PL::E, P = PL::P, GC = z3_rows<N>(), TG = GC * P, R = GC * row_pitch(M);
+  static_assert(TG % 32 == 0 || TG * 3 <= 32, "component groups are whole warps");
+  const int comp = threadIdx.x / TG, t = threadIdx.x % TG;
+  const int p = t % P, g = t / P;
+  const int64_t row0 = (int64_t)blockIdx.x * GC, row = row0 + g;
   const bool ok = row < nrows;
-  RowSmem sm{smem + g * row_pitch(M)};
-#pragma unroll 1
-  for (int comp = 0; comp < 3; ++comp) {
-    const float2* src = (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * (M + 1);
-    float2 v[E];
+  float2* region = smem + comp * R;
+  const float2* src = (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * (M + 1);
+  float2 v[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-      const int k = p + P * e;
-      float2 z = make_float2(0.f, 0.f);
-      if (ok) {
-        float2 xk = src[k], xm = src[M - k];
-        if (comp == 2) {
-          const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
-          xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
-        }
-        if (k == 0) {
-          z = make_float2(xk.x + xm.x, xk.x - xm.x);
-        } else {
-          const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
-          const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
-          const float2 w = __ldg(twn + k);
-          const float2 b = cmul(d, make_float2(w.x, -w.y));
-          z = make_float2(a.x - b.y, a.y + b.x);
-        }
-      }
-      v[e] = cswap(z);
-    }
-    fft_line<M>(v, p, sm, tw);
+  for (int e = 0; e < E; ++e) {
+    const int k = p + P * e;
+    float2 z = make_float2(0.f, 0.f);
     if (ok) {
-      float* dst = out4 + row * (4 * (int64_t)N) + comp;
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const int z = 2 * (p + P * e);
-        dst[4 * z] = v[e].y * scale;
-        dst[4 * z + 4] = v[e].x * scale;
+      float2 xk = src[k], xm = src[M - k];
+      if (comp == 2) {
+        const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
+        xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
+      }
+      if (k == 0) {
+        z = make_float2(xk.x + xm.x, xk.x - xm.x);
+      } else {
+        const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
+        const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
+        const float2 w = __ldg(twn + k);
+        const float2 b = cmul(d, make_float2(w.x, -w.y));
+        z = make_float2(a.x - b.y, a.y + b.x);
       }
     }
-    if constexpr (PL::NST > 1) __syncthreads();   // the exchange buffer is reused by the next component
+    v[e] = cswap(z);
   }
+  RowSmem sm{region + g * row_pitch(M)};
+  fft_line<M>(v, p, sm, tw);
+  if constexpr (PL::NST > 1) __syncthreads();   // exchange buffers free: park the real rows in them
+  // cells (2k, 2k+1) of row g = (im, re) of the swapped result
+#pragma unroll
+  for (int e = 0; e < E; ++e) region[g * M + p + P * e] = make_float2(v[e].y * scale, v[e].x * scale);
+  __syncthreads();
+  const float* b0 = reinterpret_cast<const float*>(smem);
+  const float* b1 = reinterpret_cast<const float*>(smem + R);
+  const float* b2 = reinterpret_cast<const float*>(smem + 2 * R);
+  const int64_t left = nrows - row0;
+  const int cells = (int)(left < GC ? left : GC) * N;
+  float4* dst = out4 + row0 * N;
+  for (int i = threadIdx.x; i < cells; i += 3 * TG) dst[i] = make_float4(b0[i], b1[i], b2[i], 0.f);
 }
 
 }  // namespace fpm
