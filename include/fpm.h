@@ -189,6 +189,29 @@ int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t
 int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n,
                         const float* grad_out, float* grad_mesh, float* grad_pos);
 
+/* ---- reverse mode through a force evaluation, a run and the initial conditions ---------------
+ * (needed by BASELINE.json's C4 "backward pass: gradient of sum(final density x
+ * weight field) with respect to the initial linear modes, via adjoint paint/readout/FFT").  All need
+ * the workspace. */
+
+/* grad_pos [3][n] += coef * J_f(pos)^T v, where f = fpm_force(pos) and v [3][n] is the cotangent of
+ * the force: the direct dW/dx term of the three readouts plus the path through paint -> r2c ->
+ * transfer function -> c2r (whose transpose is its negative: the kernel is odd and imaginary). */
+int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, double coef,
+                  float* grad_pos);
+
+/* Reverse of fpm_nbody.  traj: DEVICE [(n_steps+1)][3][n] as stored by fpm_nbody for the same HOST
+ * a_stages.  grad_pos / grad_mom: DEVICE [3][n]; on entry dL/d(final pos, final mom), on return
+ * dL/d(initial pos, initial mom) (updated in place).  The forward force meshes of every step are
+ * recomputed from traj. */
+int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n_steps,
+                  float* grad_pos, float* grad_mom);
+
+/* Reverse of fpm_lpt_init.  grad_pos / grad_mom: DEVICE [3][np^3] (read only); grad_delta: DEVICE
+ * [np^3] = dL/d(delta_lin) (overwritten).  delta_lin, a0, order as in the forward call. */
+int fpm_lpt_init_vjp(fpm_ctx* ctx, const float* delta_lin, double a0, int order,
+                     const float* grad_pos, const float* grad_mom, float* grad_delta);
+
 /* ---- measurement hooks -------------------------------------------------------------------- */
 /* Per-kernel CUDA-event timing on the context's stream (off by default).  fpm_profile_read
  * synchronises the recorded events; kernel_id runs over 0 .. until FPM_EINVAL is returned.

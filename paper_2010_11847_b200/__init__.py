@@ -70,6 +70,9 @@ def _load():
         "fpm_profile_read": (i32, [vp, i32, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(dbl),
                                    ctypes.POINTER(i64)]),
         "fpm_launch_count": (i64, [vp]),
+        "fpm_force_vjp": (i32, [vp, vp, i64, vp, dbl, vp]),
+        "fpm_nbody_vjp": (i32, [vp, vp, ctypes.POINTER(dbl), i32, vp, vp]),
+        "fpm_lpt_init_vjp": (i32, [vp, vp, dbl, i32, vp, vp, vp]),
         "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
         "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
     }
@@ -309,3 +312,24 @@ class FPM:
         self._check(_lib.fpm_readout_adjoint(self._h, _dev(mesh), _dev(pos), n, _dev(grad_out),
                                              _dev(gm), _dev(gpos)))
         return gm, gpos
+
+    # ---- reverse mode --------------------------------------------------
+    def force_vjp(self, pos, v, coef=1.0, grad_pos=None):
+        """grad_pos += coef * J_f(pos)^T v for f = force(pos); returns grad_pos [3][n]."""
+        n = pos.shape[1]
+        g = grad_pos if grad_pos is not None else torch.zeros(3, n, dtype=torch.float32, device=self.device)
+        self._check(_lib.fpm_force_vjp(self._h, _dev(pos), n, _dev(v), float(coef), _dev(g)))
+        return g
+
+    def nbody_vjp(self, traj, stages, grad_pos, grad_mom):
+        """Cotangents of the final (pos, mom) -> of the initial (pos, mom), in place."""
+        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+        self._check(_lib.fpm_nbody_vjp(self._h, _dev(traj), st, len(stages) - 1, _dev(grad_pos),
+                                       _dev(grad_mom)))
+        return grad_pos, grad_mom
+
+    def lpt_init_vjp(self, delta_lin, a0, order, grad_pos, grad_mom):
+        out = self._empty(self.np_side, self.np_side, self.np_side)
+        self._check(_lib.fpm_lpt_init_vjp(self._h, _dev(delta_lin), a0, order, _dev(grad_pos),
+                                          _dev(grad_mom), _dev(out)))
+        return out

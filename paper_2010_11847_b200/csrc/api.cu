@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "fpm_internal.h"
 
@@ -124,6 +125,35 @@ int pm_step(fpm_ctx* ctx, const Workspace& w, float* pos, float* mom, int64_t n,
   else
     FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
                                      (float)dfac, order_of(ctx, n), ctx->stream));
+  return FPM_OK;
+}
+
+// gx += coef * J_f(pos)^T v, f = the force evaluation of force_meshes + readout.
+int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, const float* v, double coef,
+              float* gx) {
+  const int ng = ctx->cfg.ng;
+  cudaStream_t s = ctx->stream;
+  Profiler* pr = &ctx->prof;
+  const ParticleOrder ord = order_of(ctx, n);
+  const double sc = 1.5 * ctx->cfg.omega_m;
+  // forward force meshes F_d at pos (recomputed, not stored)
+  const int rc = force_meshes(ctx, w, pos, n, false);
+  if (rc != FPM_OK) return rc;
+  // f_d = readout(F_d, pos): direct dW/dx term
+  { ProfScope sc2(pr, K_READOUT_GRAD);
+    FPM_CUDA(ctx, readout3_grad_accum(w.F[0], w.F[1], w.F[2], pos, v, (float)coef, n, ng, gx, s)); }
+  // ... and the cotangent of the meshes: Fbar_d = paint(pos, mass = v_d)
+  for (int d = 0; d < 3; ++d) {
+    { ProfScope sc2(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.rho, true, ord, s)); }
+    FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.fk[d], s, pr));
+  }
+  // rho_bar = sum_d M_d^T Fbar_d = -sum_d M_d Fbar_d
+  { ProfScope sc2(pr, K_GREEN);
+    FPM_CUDA(ctx, apply_force_kernel_transpose(ctx->kt_g, w.fk[0], w.fk[1], w.fk[2], (float)(coef * sc), w.dk, s)); }
+  FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.dk, w.F[0], s, pr));
+  // rho = paint(pos, m): cotangent of pos = m sum_c rho_bar[c] dW/dx
+  ProfScope sc2(pr, K_READOUT_GRAD);
+  FPM_CUDA(ctx, readout_grad(w.F[0], pos, nullptr, particle_mass(ctx), n, ng, gx, nullptr, s, true));
   return FPM_OK;
 }
 
@@ -417,6 +447,122 @@ int fpm_pm_step_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, flo
   FPM_CUDA(ctx, cudaMemcpyAsync(h_pos, d_pos, bytes, cudaMemcpyDeviceToHost, s));
   FPM_CUDA(ctx, cudaMemcpyAsync(h_mom, d_mom, bytes, cudaMemcpyDeviceToHost, s));
   FPM_CUDA(ctx, cudaStreamSynchronize(s));
+  return FPM_OK;
+}
+
+int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, double coef,
+                  float* grad_pos) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((pos && v && grad_pos) || n == 0), "fpm_force_vjp: bad arguments");
+  FPM_REQUIRE(ctx, std::isfinite(coef), "fpm_force_vjp: non-finite coefficient");
+  FPM_NEED_WS(ctx);
+  return force_vjp(ctx, carve(ctx), pos, n, v, coef, grad_pos);
+}
+
+int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n_steps,
+                  float* grad_pos, float* grad_mom) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, traj && a_stages && grad_pos && grad_mom && n_steps >= 0, "fpm_nbody_vjp: bad arguments");
+  for (int j = 0; j <= n_steps; ++j)
+    FPM_REQUIRE(ctx, a_stages[j] > 0.0, "fpm_nbody_vjp: scale factors must be positive");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  const int np = ctx->cfg.np;
+  const int64_t n = (int64_t)np * np * np;
+  const double om = ctx->cfg.omega_m;
+  const int fm = ctx->cfg.factor_mode;
+  // the same merged factors as fpm_nbody: step j is  p += kf_j f(x_j);  x = wrap(x + dr_j p)
+  std::vector<double> kf(n_steps + 1), dr(n_steps + 1);
+  double pending = 0.0;
+  for (int j = 0; j <= n_steps; ++j) {
+    kf[j] = pending; dr[j] = 0.0;
+    if (j < n_steps) {
+      const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
+      kf[j] += kick_factor(om, ai, ai, ah, fm);
+      dr[j] = drift_factor(om, ai, ah, af, fm);
+      pending = kick_factor(om, ah, af, af, fm);
+    }
+  }
+  for (int j = n_steps; j >= 0; --j) {
+    // x' = wrap(x + dr p'):  p'_bar += dr x'_bar   (wrap has unit derivative)
+    if (dr[j] != 0.0) {
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, axpy(grad_mom, grad_pos, (float)dr[j], 3 * n, ctx->stream));
+    }
+    // p' = p + kf f(x_j):  x_bar += kf J_f(x_j)^T p'_bar
+    if (kf[j] != 0.0) {
+      const int rc = force_vjp(ctx, w, traj + (int64_t)j * 3 * n, n, grad_mom, kf[j], grad_pos);
+      if (rc != FPM_OK) return rc;
+    }
+  }
+  return FPM_OK;
+}
+
+int fpm_lpt_init_vjp(fpm_ctx* ctx, const float* delta_lin, double a0, int order,
+                     const float* grad_pos, const float* grad_mom, float* grad_delta) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, delta_lin && grad_pos && grad_mom && grad_delta, "fpm_lpt_init_vjp: null pointer");
+  FPM_REQUIRE(ctx, order == 1 || order == 2, "fpm_lpt_init_vjp: order must be 1 or 2");
+  FPM_REQUIRE(ctx, a0 > 0.0, "fpm_lpt_init_vjp: a0 must be positive");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  cudaStream_t s = ctx->stream;
+  Profiler* pr = &ctx->prof;
+  const int np = ctx->cfg.np, bfac = ctx->cfg.ng / np;
+  const int64_t n3 = (int64_t)np * np * np;
+  const GrowthOut g = growth(ctx->cfg.omega_m, a0);
+  const double pre = a0 * a0 * g.E;
+  float2 *dk = w.dk, *tk = w.fk[0], *acck = w.fk[1];
+  float* bar = reinterpret_cast<float*>(w.fk[2]);
+  float* sbar = w.rho;
+  // x = q B + (D1 psi1 + D2 psi2) B,  p = a^2 E (f1 D1 psi1 + f2 D2 psi2) B
+  // psi1_d = T[i k_d / k^2] delta  ->  delta_bar_k += (-i k_d / k^2) psi1bar_d,k
+  for (int d = 0; d < 3; ++d) {
+    ctx->prof.launches += 1;
+    FPM_CUDA(ctx, lincomb2(bar, grad_pos + d * n3, (float)(bfac * g.D1), grad_mom + d * n3,
+                           (float)(bfac * pre * g.f1 * g.D1), n3, s));
+    FPM_CUDA(ctx, fft_r2c(ctx->fft_p, bar, tk, s, pr));
+    ctx->prof.launches += 1;
+    FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, tk, acck, d, -1, 1.f, s, d > 0));
+  }
+  if (order == 2) {
+    // psi2_d = T[-i k_d / k^2] S  ->  S_bar_k = sum_d (+i k_d / k^2) psi2bar_d,k
+    for (int d = 0; d < 3; ++d) {
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lincomb2(bar, grad_pos + d * n3, (float)(bfac * g.D2), grad_mom + d * n3,
+                             (float)(bfac * pre * g.f2 * g.D2), n3, s));
+      FPM_CUDA(ctx, fft_r2c(ctx->fft_p, bar, tk, s, pr));
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, tk, dk, d, -1, -1.f, s, d > 0));
+    }
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_p, dk, sbar, s, pr));
+    // S = sum_{i<j} (phi,ii phi,jj - phi,ij^2), phi,ij = T[k_i k_j / k^2] delta (real, even: self-adjoint)
+    FPM_CUDA(ctx, fft_r2c(ctx->fft_p, delta_lin, dk, s, pr));
+    for (int c = 0; c < 3; ++c) {
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, c, c, 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, w.F[c], s, pr));
+    }
+    for (int c = 0; c < 3; ++c) {
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_phibar(bar, sbar, w.F[(c + 1) % 3], w.F[(c + 2) % 3], n3, s));
+      FPM_CUDA(ctx, fft_r2c(ctx->fft_p, bar, tk, s, pr));
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, tk, acck, c, c, 1.f, s, true));
+    }
+    const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+    for (auto& pq : pairs) {
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, dk, tk, pq[0], pq[1], 1.f, s));
+      FPM_CUDA(ctx, fft_c2r(ctx->fft_p, tk, w.F[0], s, pr));
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_phibar(bar, sbar, w.F[0], nullptr, n3, s));
+      FPM_CUDA(ctx, fft_r2c(ctx->fft_p, bar, tk, s, pr));
+      ctx->prof.launches += 1;
+      FPM_CUDA(ctx, lpt_spectral(ctx->kt_p, tk, acck, pq[0], pq[1], 1.f, s, true));
+    }
+  }
+  FPM_CUDA(ctx, fft_c2r(ctx->fft_p, acck, grad_delta, s, pr));
   return FPM_OK;
 }
 

@@ -94,8 +94,14 @@ cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, floa
 cudaError_t readout3(const float* fx, const float* fy, const float* fz, const float* pos, int64_t n,
                      int ng, float* out3, const ParticleOrder& ord, cudaStream_t s);
 // gradient of the CIC sum w.r.t. the position, times scale_p (mass[p] or vbar[p] or constant)
+// accumulate: out3 += instead of out3 =
 cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale, float scale_const,
-                         int64_t n, int ng, float* out3, float* out_value, cudaStream_t s);
+                         int64_t n, int ng, float* out3, float* out_value, cudaStream_t s,
+                         bool accumulate = false);
+// gx[e][p] += coef * sum_d v[d][p] * sum_c F_d[c] dW/dx_e  (direct term of the force VJP, R12)
+cudaError_t readout3_grad_accum(const float* f0, const float* f1, const float* f2, const float* pos,
+                                const float* v, float coef, int64_t n, int ng, float* gx,
+                                cudaStream_t s);
 
 // ---- particle updates (particles.cu) -----------------------------------------------------------
 cudaError_t kick(float* mom, const float* force, int64_t n3, float fac, cudaStream_t s);
@@ -110,8 +116,18 @@ cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz
 cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float scale, float2* fkx,
                                float2* fky, float2* fkz, cudaStream_t s);
 // out = mult(k) in, mult = sign * (a == b ? -k_a^2 : (i k_a)(b >= 0 ? i k_b : 1)) * (-1/k^2)
+// accumulate: out += instead of out =
 cudaError_t lpt_spectral(const KernelTables& kt, const float2* in, float2* out, int a, int b,
-                         float sign, cudaStream_t s);
+                         float sign, cudaStream_t s, bool accumulate = false);
+// backward pass: out_k = - sum_d (i scale g_d / K^2) f_d,k  (= sum_d M_d^T)
+cudaError_t apply_force_kernel_transpose(const KernelTables& kt, const float2* f0, const float2* f1,
+                                         const float2* f2, float scale, float2* out, cudaStream_t s);
+cudaError_t axpy(float* y, const float* x, float a, int64_t n, cudaStream_t s);            // y += a x
+cudaError_t lincomb2(float* out, const float* a, float ca, const float* b, float cb, int64_t n,
+                     cudaStream_t s);                                                        // ca a + cb b
+// out = sbar (pa + pb), or -2 sbar pa when pb == nullptr (2LPT product rule)
+cudaError_t lpt_phibar(float* out, const float* sbar, const float* pa, const float* pb, int64_t n,
+                       cudaStream_t s);
 cudaError_t lpt_displace(const float* psi, int np, int bfac, int axis, float dcoef, float vcoef,
                          bool first, float* pos_d, float* mom_d, cudaStream_t s);
 cudaError_t lpt_wrap(float* pos, int64_t n3, int ng, cudaStream_t s);

@@ -41,7 +41,7 @@ force_kernel_rows(const float2* __restrict__ dk, int n, const float* __restrict_
 __global__ void __launch_bounds__(kThreads)
 lpt_spectral_rows(const float2* __restrict__ in, float2* __restrict__ out, int n,
                   const float* __restrict__ kv, const float* __restrict__ kv0, int a, int b,
-                  float sign) {
+                  float sign, int accumulate) {
   const int nzh = n / 2 + 1;
   const int x = blockIdx.x / n, y = blockIdx.x % n;
   const int64_t row = (int64_t)blockIdx.x * nzh;
@@ -64,7 +64,30 @@ lpt_spectral_rows(const float2* __restrict__ in, float2* __restrict__ out, int n
       const float m = __ldg(kv0 + idx[a]) * inv;                          // i ka
       r = make_float2(-v.y * m, v.x * m);
     }
+    if (accumulate) { const float2 o = out[row + z]; r.x += o.x; r.y += o.y; }
     out[row + z] = r;
+  }
+}
+
+// Transpose of force_kernel_rows: the mesh-to-mesh operator
+// M_d = c2r o (i s g_d / K^2) o r2c is a real convolution with an odd kernel, so M_d^T = -M_d and
+// rho_bar_k = - sum_d (i s g_d / K^2) Fbar_d,k.
+__global__ void __launch_bounds__(kThreads)
+force_kernel_transpose_rows(const float2* __restrict__ f0, const float2* __restrict__ f1,
+                            const float2* __restrict__ f2, int n, const float* __restrict__ lap,
+                            const float* __restrict__ grad, float scale, float2* __restrict__ out) {
+  const int nzh = n / 2 + 1;
+  const int x = blockIdx.x / n, y = blockIdx.x % n;
+  const float lxy = __ldg(lap + x) + __ldg(lap + y);
+  const float gx = __ldg(grad + x), gy = __ldg(grad + y);
+  const int64_t row = (int64_t)blockIdx.x * nzh;
+  for (int z = threadIdx.x; z < nzh; z += blockDim.x) {
+    const float k2 = lxy + __ldg(lap + z);
+    const float inv = (blockIdx.x == 0 && z == 0) ? 0.f : -scale / k2;
+    const float gz = __ldg(grad + z);
+    const float2 a = f0[row + z], b = f1[row + z], c = f2[row + z];
+    const float re = gx * a.x + gy * b.x + gz * c.x, im = gx * a.y + gy * b.y + gz * c.y;
+    out[row + z] = make_float2(-im * inv, re * inv);    // i (re + i im) inv
   }
 }
 
@@ -107,6 +130,30 @@ lpt_source_kernel(float* __restrict__ s, const float* __restrict__ a, const floa
     else if (mode == 1) s[i] += (a[i] + b[i]) * c[i];
     else s[i] -= a[i] * a[i];
   }
+}
+
+// y += a x
+__global__ void __launch_bounds__(256)
+axpy_kernel(float* __restrict__ y, const float* __restrict__ x, float a, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    y[i] = fmaf(a, x[i], y[i]);
+}
+
+// out = ca a + cb b
+__global__ void __launch_bounds__(256)
+lincomb2_kernel(float* __restrict__ out, const float* __restrict__ a, float ca,
+                const float* __restrict__ b, float cb, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    out[i] = ca * a[i] + cb * b[i];
+}
+
+// cotangent of a second-derivative field of the 2LPT source S (product rule):
+// diagonal: out = sbar (pa + pb) ;  off-diagonal (pb == nullptr): out = -2 sbar pa
+__global__ void __launch_bounds__(256)
+lpt_phibar_kernel(float* __restrict__ out, const float* __restrict__ sbar, const float* __restrict__ pa,
+                  const float* __restrict__ pb, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    out[i] = pb ? sbar[i] * (pa[i] + pb[i]) : -2.f * sbar[i] * pa[i];
 }
 
 inline unsigned grid_for(int64_t n) {
@@ -165,9 +212,33 @@ cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float s
 }
 
 cudaError_t lpt_spectral(const KernelTables& kt, const float2* in, float2* out, int a, int b,
-                         float sign, cudaStream_t s) {
+                         float sign, cudaStream_t s, bool accumulate) {
   lpt_spectral_rows<<<(unsigned)(kt.n * kt.n), kThreads, 0, s>>>(in, out, kt.n, kt.kvec, kt.kvec0, a,
-                                                                b, sign);
+                                                                b, sign, accumulate ? 1 : 0);
+  return cudaGetLastError();
+}
+
+cudaError_t apply_force_kernel_transpose(const KernelTables& kt, const float2* f0, const float2* f1,
+                                         const float2* f2, float scale, float2* out, cudaStream_t s) {
+  force_kernel_transpose_rows<<<(unsigned)(kt.n * kt.n), kThreads, 0, s>>>(f0, f1, f2, kt.n, kt.lap,
+                                                                          kt.grad, scale, out);
+  return cudaGetLastError();
+}
+
+cudaError_t axpy(float* y, const float* x, float a, int64_t n, cudaStream_t s) {
+  axpy_kernel<<<grid_for(n), 256, 0, s>>>(y, x, a, n);
+  return cudaGetLastError();
+}
+
+cudaError_t lincomb2(float* out, const float* a, float ca, const float* b, float cb, int64_t n,
+                     cudaStream_t s) {
+  lincomb2_kernel<<<grid_for(n), 256, 0, s>>>(out, a, ca, b, cb, n);
+  return cudaGetLastError();
+}
+
+cudaError_t lpt_phibar(float* out, const float* sbar, const float* pa, const float* pb, int64_t n,
+                       cudaStream_t s) {
+  lpt_phibar_kernel<<<grid_for(n), 256, 0, s>>>(out, sbar, pa, pb, n);
   return cudaGetLastError();
 }
 

@@ -98,17 +98,17 @@ inline bool brick_ok(int64_t n, int np) {
 }
 
 // ---- paint: direct reductions --------------------------------------------------------------------
-__device__ __forceinline__ void deposit_global(float* __restrict__ mesh, int64_t g, const Cic& c,
+__device__ __forceinline__ void deposit_global(float* __restrict__ mesh, int g, const Cic& c,
                                                float m) {
   const float wx[2] = {m * (1.f - c.t[0]), m * c.t[0]};
   const float wy[2] = {1.f - c.t[1], c.t[1]};
   const float wz[2] = {1.f - c.t[2], c.t[2]};
-  const int ix[2] = {c.i0[0], c.i1[0]}, iy[2] = {c.i0[1], c.i1[1]};
+  const unsigned ix[2] = {(unsigned)c.i0[0], (unsigned)c.i1[0]}, iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]};
 #pragma unroll
   for (int a = 0; a < 2; ++a)
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
-      float* row = mesh + ((int64_t)ix[a] * g + iy[b]) * g;
+      float* row = mesh + (ix[a] * (unsigned)g + iy[b]) * (unsigned)g;   // ng^3 <= 2^30
       const float w = wx[a] * wy[b];
       atomicAdd(row + c.i0[2], w * wz[0]);
       atomicAdd(row + c.i1[2], w * wz[1]);
@@ -165,14 +165,19 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   // mean displacement from the lattice sites (wrapped to [-ng/2, ng/2)) places the window
   float sx = 0.f, sy = 0.f, sz = 0.f, mmax = HAS_MASS ? 0.f : fabsf(mass_const);
   const float qy = (float)(qy0 + warp), qz = (float)(qz0 + lane);
+  // (a sample of kMeanPlanes of the brick's x planes is enough: the window position only decides how
+  //  many particles take the slow path, never the result)
+  constexpr int kMeanPlanes = 2, kMeanStep = kPerThread / kMeanPlanes;
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
-    float dx = x[k] - (float)(qx0 + k), dy = y[k] - qy, dz = z[k] - qz;
-    int unused;
-    dx -= fng * fast_rint(dx * inv_ng, unused);
-    dy -= fng * fast_rint(dy * inv_ng, unused);
-    dz -= fng * fast_rint(dz * inv_ng, unused);
-    sx += dx; sy += dy; sz += dz;
+    if (k % kMeanStep == 0) {
+      float dx = x[k] - (float)(qx0 + k), dy = y[k] - qy, dz = z[k] - qz;
+      int unused;
+      dx -= fng * fast_rint(dx * inv_ng, unused);
+      dy -= fng * fast_rint(dy * inv_ng, unused);
+      dz -= fng * fast_rint(dz * inv_ng, unused);
+      sx += dx; sy += dy; sz += dz;
+    }
     if (HAS_MASS) mmax = fmaxf(mmax, fabsf(m[k]));
   }
 #pragma unroll
@@ -190,7 +195,7 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
     sx += red[0][i]; sy += red[1][i]; sz += red[2][i];
     if (HAS_MASS) mmax = fmaxf(mmax, red[3][i]);
   }
-  constexpr float inv_cnt = 1.f / (float)kBrick;
+  constexpr float inv_cnt = 1.f / (float)(kBrickThreads * kMeanPlanes);
   int mx, my, mz;
   fast_floor(sx * inv_cnt, mx);
   fast_floor(sy * inv_cnt, my);
@@ -268,8 +273,8 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
       any = !(v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f);
     }
     if (any) {
-      const int gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
-      atomicAdd(reinterpret_cast<float4*>(mesh + ((int64_t)gx * ng + gy) * ng + gz), v);
+      const unsigned gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
+      atomicAdd(reinterpret_cast<float4*>(mesh + ((gx * (unsigned)ng + gy) * (unsigned)ng + gz)), v);
     }
     kz += dKz; ky += dKy; kx += dKx;
     if (kz >= WZ4) { kz -= WZ4; ky += 1; }
@@ -474,7 +479,7 @@ rkd_pipelined_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
 __global__ void __launch_bounds__(kThreads)
 readout_grad_kernel(const float* __restrict__ mesh, const float* __restrict__ pos,
                     const float* __restrict__ scale, float scale_const, int64_t n, int ng,
-                    float* __restrict__ out3, float* __restrict__ out_value) {
+                    float* __restrict__ out3, float* __restrict__ out_value, int accumulate) {
   const int64_t g = ng;
   const int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   if (p >= n) return;
@@ -500,10 +505,54 @@ readout_grad_kernel(const float* __restrict__ mesh, const float* __restrict__ po
       }
     }
   const float s = scale ? ld_stream(scale + p) : scale_const;
-  out3[p] = s * gx;
-  out3[n + p] = s * gy;
-  out3[2 * n + p] = s * gz;
+  if (accumulate) {
+    out3[p] = fmaf(s, gx, out3[p]);
+    out3[n + p] = fmaf(s, gy, out3[n + p]);
+    out3[2 * n + p] = fmaf(s, gz, out3[2 * n + p]);
+  } else {
+    out3[p] = s * gx;
+    out3[n + p] = s * gy;
+    out3[2 * n + p] = s * gz;
+  }
   if (out_value) out_value[p] = val;
+}
+
+// Direct term of the force VJP: the force f_d = readout(F_d, x) depends on x
+// through the CIC weights;  gx[e][p] += coef * sum_d v[d][p] * sum_c F_d[c] dW/dx_e.
+__global__ void __launch_bounds__(kThreads)
+readout3_grad_accum_kernel(const float* __restrict__ f0, const float* __restrict__ f1,
+                           const float* __restrict__ f2, const float* __restrict__ pos,
+                           const float* __restrict__ v, float coef, int64_t n, int ng,
+                           float* __restrict__ gx) {
+  const int64_t p = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+  if (p >= n) return;
+  const unsigned g = ng;
+  const Cic c = cic_of(ld_stream(pos + p), ld_stream(pos + n + p), ld_stream(pos + 2 * n + p), ng - 1);
+  const float v0 = ld_stream(v + p), v1 = ld_stream(v + n + p), v2 = ld_stream(v + 2 * n + p);
+  const float wx[2] = {1.f - c.t[0], c.t[0]};
+  const float wy[2] = {1.f - c.t[1], c.t[1]};
+  const float wz[2] = {1.f - c.t[2], c.t[2]};
+  const float sg[2] = {-1.f, 1.f};
+  const unsigned ix[2] = {(unsigned)c.i0[0], (unsigned)c.i1[0]}, iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]},
+                 iz[2] = {(unsigned)c.i0[2], (unsigned)c.i1[2]};
+  float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const unsigned row = (ix[a] * g + iy[b]) * g;
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const unsigned i = row + iz[e];
+        const float f = v0 * __ldg(f0 + i) + v1 * __ldg(f1 + i) + v2 * __ldg(f2 + i);
+        ax = fmaf(f, sg[a] * wy[b] * wz[e], ax);
+        ay = fmaf(f, wx[a] * sg[b] * wz[e], ay);
+        az = fmaf(f, wx[a] * wy[b] * sg[e], az);
+      }
+    }
+  gx[p] = fmaf(coef, ax, gx[p]);
+  gx[n + p] = fmaf(coef, ay, gx[n + p]);
+  gx[2 * n + p] = fmaf(coef, az, gx[2 * n + p]);
 }
 
 inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kThreads - 1) / kThreads); }
@@ -588,10 +637,19 @@ cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz
 }
 
 cudaError_t readout_grad(const float* mesh, const float* pos, const float* scale, float scale_const,
-                         int64_t n, int ng, float* out3, float* out_value, cudaStream_t s) {
+                         int64_t n, int ng, float* out3, float* out_value, cudaStream_t s,
+                         bool accumulate) {
   if (n == 0) return cudaSuccess;
   readout_grad_kernel<<<blocks_for(n), kThreads, 0, s>>>(mesh, pos, scale, scale_const, n, ng, out3,
-                                                         out_value);
+                                                         out_value, accumulate ? 1 : 0);
+  return cudaGetLastError();
+}
+
+cudaError_t readout3_grad_accum(const float* f0, const float* f1, const float* f2, const float* pos,
+                                const float* v, float coef, int64_t n, int ng, float* gx,
+                                cudaStream_t s) {
+  if (n == 0) return cudaSuccess;
+  readout3_grad_accum_kernel<<<blocks_for(n), kThreads, 0, s>>>(f0, f1, f2, pos, v, coef, n, ng, gx);
   return cudaGetLastError();
 }
 
