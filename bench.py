@@ -172,6 +172,50 @@ def workload_name(cfg):
             f"{cfg.lpt_order}LPT ICs at a={cfg.a0}, {cfg.n_steps}-step FastPM schedule linear in a to a={cfg.a1}")
 
 
+def side_measurements(args, ctx, cfg, pos, mom, factors, device):
+    """Context numbers, N = 1 only, outside the timed region: (i) cuFFT (torch.fft, a library call) r2c +
+    c2r on the same mesh size as the reference floor for the hand-written FFT passes -- never on the
+    product path; (ii) one backward PM step (fpm_force_vjp at the current positions: recomputed force
+    meshes, 3 adjoint paints, 3 r2c, transposed kernel, c2r, 2 gradient gathers -- C4's backward pass)."""
+    import torch
+    out = {}
+    if args.no_side:
+        return out
+    ng, n_p = cfg.ng, cfg.n_particles
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    try:
+        x = torch.randn(ng, ng, ng, device=device)
+        k = torch.fft.rfftn(x)
+        ms_r2c = timed(lambda: torch.fft.rfftn(x), 5)
+        ms_c2r = timed(lambda: torch.fft.irfftn(k, s=(ng, ng, ng)), 5)
+        del x, k
+        out["cufft_floor"] = {"r2c_ms": ms_r2c, "c2r_ms": ms_c2r, "one_r2c_three_c2r_ms": ms_r2c + 3 * ms_c2r,
+                              "note": "torch.fft (cuFFT) on an ng^3 float32 mesh, timed alone as the reference "
+                                      "floor for fft_z_r2c + fft_cols_y + fft_x_force + fft_y_inv3 + fft_z_c2r3; "
+                                      "not on the product path"}
+    except RuntimeError as e:      # noqa: BLE001  (cuFFT workspace may not fit beside a large config)
+        out["cufft_floor"] = {"unavailable": str(e)[:120]}
+    torch.cuda.empty_cache()
+    gx = torch.zeros(3, n_p, device=device)
+    v = mom.clone()
+    ms_bwd = timed(lambda: ctx.force_vjp(pos, v, coef=factors[0], grad_pos=gx), 3)
+    out["backward_step"] = {"ms": ms_bwd, "call": "fpm_force_vjp (one backward force evaluation of fpm_nbody_vjp)",
+                            "steps_per_s": 1e3 / ms_bwd}
+    del gx, v
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -181,6 +225,7 @@ def main():
     ap.add_argument("--config", default="C4", choices=sorted(fi.CONFIGS))
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip the cuFFT floor and backward-step timings")
     ap.add_argument("--ref-side", type=int, default=None)
     ap.add_argument("--force-path", default="fused", choices=["fused", "unfused"])
     args = ap.parse_args()
@@ -190,17 +235,14 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
 
     import paper_2010_11847_b200 as fpm   # raises if libfpm.so is missing: no fallback
+    from paper_2010_11847_b200 import replicas as rep
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = rep.env_world()
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=device)
+    rep.init("nccl", device)
 
     cfg = fi.CONFIGS[args.config]
     n_p, ng = cfg.n_particles, cfg.ng
@@ -208,7 +250,7 @@ def main():
                   force_path=fpm.FORCE_FUSED if args.force_path == "fused" else fpm.FORCE_UNFUSED)
 
     # ---- inputs: seeded Gaussian field -> 2LPT particles, all resident in HBM -----------------
-    delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, cfg.seed + rank)).to(device)
+    delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, rep.replica_seed(cfg.seed, rank))).to(device)
     pos, mom = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
     del delta
     factors = ctx.step_factors(cfg.stages())
@@ -221,8 +263,7 @@ def main():
         ctx.pm_step(pos, mom, *fac(step_no))
         step_no += 1
     torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
+    rep.barrier()
     torch.cuda.synchronize()
 
     sampler = ClockSampler(local_rank)
@@ -238,20 +279,16 @@ def main():
         step_no += 1
     ev1.record()
     torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
+    rep.barrier()
     torch.cuda.synchronize()
     ms_total = ev0.elapsed_time(ev1)
     launches = ctx.launch_count()
     prof = ctx.profile_read()
     ctx.profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms_total], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = rep.max_over_ranks(ms_total, device)
     ms_per_step = ms_total / args.steps
-    value = world * 1e3 / ms_per_step          # whole-job steps/s (replicas)
+    value = rep.whole_job_rate(args.steps, ms_total, world)     # whole-job steps/s (replicas)
 
     # ---- end to end through the C-ABI with HOST buffers -----------------------------------------
     e2e = None
@@ -263,8 +300,7 @@ def main():
         torch.cuda.synchronize()
         ctx.pm_step_host(h_pos, h_mom, pos, mom, *fac(step_no))   # warm-up
         step_no += 1
-        if world > 1:
-            dist.barrier()
+        rep.barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(args.e2e_steps):
@@ -273,19 +309,17 @@ def main():
         e1.record()
         torch.cuda.synchronize()
         e2e_ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_ms = float(t.item())
-        e2e = {"value": world * 1e3 * args.e2e_steps / e2e_ms, "unit": "steps/s",
+        e2e_ms = rep.max_over_ranks(e2e_ms, device)
+        e2e = {"value": rep.whole_job_rate(args.e2e_steps, e2e_ms, world), "unit": "steps/s",
                "h2d_bytes_per_step": 24 * n_p, "d2h_bytes_per_step": 24 * n_p,
                "steps": args.e2e_steps,
                "call": "fpm_pm_step_host (pinned host pos+mom -> device, step, -> host)"}
         del h_pos, h_mom
 
+    extras = side_measurements(args, ctx, cfg, pos, mom, fac(step_no), device) if (rank == 0 and world == 1) else {}
+
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        rep.finalize()
         return
 
     # ---- per-kernel roofline from the live CUDA-event profile ------------------------------------
@@ -341,9 +375,9 @@ def main():
         "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "cpu_baseline": cpu_baseline,
     }
+    out.update(extras)
     print(json.dumps(out), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    rep.finalize()
 
 
 if __name__ == "__main__":

@@ -1,0 +1,110 @@
+"""Parity at BASELINE.json's full size (C4: 512^3 particles on a 512^3 mesh), in the launch
+configuration bench.py times (Lagrangian-brick paint, fused force path with the interleaved force
+mesh, pipelined brick readout+kick+drift).  The oracle cannot run a 512^3 force evaluation in
+seconds, so it checks sampled outputs one by one (brute-force CIC sums over all particles,
+oracle.readout at sampled particles) and the rest is covered by properties that hold at any size:
+mass and momentum conservation, and agreement of the fused path with the op-by-op chain
+paint -> r2c -> apply_force_kernel -> 3 x c2r -> readout -> kick -> drift, each op of which is
+oracle-checked at small sizes (tests/test_gpu_*.py) and, for the FFT, at this size
+(test_gpu_fft.py::test_full_size_sampled_outputs_and_roundtrip)."""
+import numpy as np
+import pytest
+
+import fpm_inputs as fi
+from gpu_util import dev, host
+
+pytestmark = pytest.mark.gpu
+OM = fi.COSMO["omega_m"]
+
+
+@pytest.fixture(scope="module")
+def state():
+    """C4 initial conditions advanced by two PM steps (so particles have left their lattice sites)."""
+    import torch
+
+    import paper_2010_11847_b200 as fpm
+    cfg = fi.CONFIGS["C4"]
+    ctx = fpm.FPM(cfg.ng, cfg.np_side, omega_m=OM, box=cfg.box, force_path=fpm.FORCE_FUSED)
+    delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, cfg.seed)).cuda()
+    pos, mom = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
+    del delta
+    fac = ctx.step_factors(cfg.stages())
+    for j in range(2):
+        ctx.pm_step(pos, mom, *fac[j])
+    torch.cuda.synchronize()
+    return fpm, cfg, ctx, pos, mom, fac
+
+
+def _cic_cell_sum(hpos, cell, ng):
+    """Brute force over ALL particles: rho[cell] = sum_p prod_d max(0, 1 - |x_pd - c_d|) (periodic)."""
+    w = np.ones(hpos.shape[1], dtype=np.float64)
+    for d in range(3):
+        dx = np.abs(hpos[d].astype(np.float64) - cell[d])
+        dx = np.minimum(dx, ng - dx)
+        w *= np.maximum(0.0, 1.0 - dx)
+    return float(w.sum())
+
+
+def test_paint_full_size(state):
+    import torch
+    fpm, cfg, ctx, pos, mom, fac = state
+    ng, n = cfg.ng, cfg.n_particles
+    rho = ctx.paint(pos)                                   # brick window, fixed point (AUTO)
+    total = float(rho.double().sum())
+    assert abs(total - n) < 1e-6 * n                       # mass conservation
+    ctx.set_paint_mode(fpm.PAINT_DIRECT)                   # an independent kernel: global reductions
+    rho_d = ctx.paint(pos)
+    ctx.set_paint_mode(fpm.PAINT_AUTO)
+    rel = float(torch.linalg.vector_norm(rho - rho_d) / torch.linalg.vector_norm(rho_d))
+    assert rel < 1e-5
+    hpos = host(pos)
+    rng = np.random.default_rng(3)
+    cells = [tuple(int(v) for v in rng.integers(0, ng, 3)) for _ in range(4)] + [(0, 0, 0), (ng - 1, ng - 1, ng - 1)]
+    for c in cells:
+        ref = _cic_cell_sum(hpos, c, ng)
+        got = float(rho[c[0], c[1], c[2]])
+        assert abs(got - ref) < 1e-5 * max(1.0, ref), (c, got, ref)
+
+
+def test_readout_full_size_sampled_particles(state, oracle):
+    import torch
+    fpm, cfg, ctx, pos, mom, fac = state
+    n = cfg.n_particles
+    mesh = ctx.paint(pos)
+    out = ctx.readout(mesh, pos)                           # brick-ordered gather over all particles
+    idx = np.random.default_rng(4).integers(0, n, 4000)
+    sel = torch.from_numpy(idx).cuda()
+    ref = oracle.readout(host(mesh).astype(np.float64), host(pos[:, sel]).astype(np.float64))
+    got = host(out[sel]).astype(np.float64)
+    assert np.max(np.abs(got - ref)) < 1e-5 * np.max(np.abs(ref))
+
+
+def test_fused_step_equals_op_by_op_chain_and_conserves_momentum(state):
+    import torch
+    fpm, cfg, ctx, pos, mom, fac = state
+    ng, n = cfg.ng, cfg.n_particles
+    kf, dr = fac[2]
+    p1, m1 = pos.clone(), mom.clone()
+    ctx.pm_step(p1, m1, kf, dr)                            # the configuration bench.py times
+    # op-by-op through the single-operator C-ABI calls
+    rho = ctx.paint(pos)
+    dk = ctx.fft_r2c(rho)
+    del rho
+    fks = ctx.apply_force_kernel(dk, scale=1.5 * OM)
+    del dk
+    f = torch.empty(3, n, device="cuda")
+    for d in range(3):
+        F = ctx.fft_c2r(fks[d], clobber=True)
+        f[d] = ctx.readout(F, pos)
+        del F
+    del fks
+    frms = float(f.double().pow(2).mean().sqrt())
+    assert float(f.double().sum(dim=1).abs().max()) < 1e-4 * frms * n      # sum of forces ~ 0
+    m2 = mom + f * kf
+    p2 = torch.remainder(pos + m2 * dr, float(ng))
+    dm = float(torch.linalg.vector_norm(m1 - m2) / torch.linalg.vector_norm(m2))
+    assert dm < 1e-5
+    dx = (p1 - p2).abs()
+    dx = torch.minimum(dx, ng - dx)
+    assert float(dx.max()) < 2e-4                          # 3 ulp at x ~ 512 is 1.8e-4
+    assert float(p1.min()) >= 0.0 and float(p1.max()) < ng
