@@ -154,12 +154,13 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   const size_t smem = Plan<N>::NST > 1 ? sizeof(float2) * N * T : 0;
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
+    constexpr int TX = xf_tile<N>();
     auto kern = fft_x_force_kernel<N>;
-    e = set_smem(kern, smem);
+    e = set_smem(kern, xf_smem_bytes<N>());
     if (e != cudaSuccess) return e;
     const int ncols = N * nzh;
-    kern<<<2 * ((ncols + T - 1) / T), threads, smem, s>>>(dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_n,
-                                                        kt.lap, kt.grad, scale);
+    kern<<<(ncols + TX - 1) / TX, TX * Plan<N>::P, xf_smem_bytes<N>(), s>>>(
+        dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_n, kt.lap, kt.grad, scale);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }

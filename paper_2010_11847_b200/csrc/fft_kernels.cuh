@@ -16,6 +16,9 @@ struct OpNone {
 };
 
 template <int N> __host__ __device__ constexpr int col_tile() { return N >= 64 ? 16 : 32; }
+// resident blocks per SM the column kernels are compiled for: at N = 512 the 64 KB tile allows three,
+// which needs <= 85 registers (the compiler otherwise settles just above and only two fit)
+template <int N> __host__ __device__ constexpr int cols_min_blocks() { return N == 512 ? 3 : 1; }
 template <int N> __host__ __device__ constexpr int z_rows() {          // lines per block on the z pass
   constexpr int P = Plan<N / 2>::P;
   return P >= 256 ? 1 : 256 / P;
@@ -25,7 +28,7 @@ template <int N> __host__ __device__ constexpr int z_rows() {          // lines 
 // grid = (ceil(ncols / T), batches); element (line i, column c) of batch b at
 //   b * batch_stride + i * line_stride + c.
 template <int N, bool INV, class LOADOP, class STOREOP>
-__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P, cols_min_blocks<N>())
 fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
                 int64_t line_stride, const float2* __restrict__ tw, LOADOP lop, STOREOP sop) {
   extern __shared__ float2 smem[];
@@ -56,24 +59,29 @@ fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
 }
 
 // Fused transfer function (Eq. 3-5) on the x axis: forward x transform of the
-// y-transformed density, times  i s / K^2  (variant 0: "A")  or  i s g(w_x) / K^2  (variant 1: "Bx"),
-// inverse x transform, all inside one block -- delta_k, and the three force spectra of the unfused
-// path, never reach HBM.  Since g(w_y) and g(w_z) are constant along x, F_y and F_z follow from A
-// by a multiplication in the y and z passes.  Block b: tile b >> 1, variant b & 1 (the two readers
-// of a tile run back to back, so the second read is an L2 hit).
+// y-transformed density, times  i s / K^2  ("A")  and  i s g(w_x) / K^2  ("Bx"), and the two inverse x
+// transforms, all inside one block -- delta_k, and the three force spectra of the unfused path, never
+// reach HBM.  Since g(w_y) and g(w_z) are constant along x, F_y and F_z follow from A by a
+// multiplication in the y and z passes.  The spectrum A is parked in a second shared-memory tile
+// while its inverse runs, so the forward transform is done once (1 forward + 2 inverse per column).
 // columns = flattened (y, kz), lines = x with stride line_stride; no normalisation here.
+// Tile of TX columns; shared memory = [exchange N*TX | parked spectrum N*TX] float2.
+template <int N> __host__ __device__ constexpr int xf_tile() { return N >= 512 ? 8 : col_tile<N>(); }
+template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
+  return sizeof(float2) * 2 * (size_t)N * xf_tile<N>();
+}
+
 template <int N>
-__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N>::P)
 fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
                    float2* __restrict__ out_bx, int ncols, int nzh, int64_t line_stride,
                    const float2* __restrict__ tw, const float* __restrict__ lap,
                    const float* __restrict__ grad, float scale) {
   extern __shared__ float2 smem[];
   using PL = Plan<N>;
-  constexpr int T = col_tile<N>(), E = PL::E, P = PL::P;
+  constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
-  const int variant = blockIdx.x & 1;
-  const int64_t col = (int64_t)(blockIdx.x >> 1) * T + c;
+  const int64_t col = (int64_t)blockIdx.x * T + c;
   const bool ok = col < ncols;
   float2 v[E];
 #pragma unroll
@@ -83,21 +91,33 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
   fft_line<N>(v, p, sm, tw);
   const int y = ok ? (int)(col / nzh) : 0, kz = ok ? (int)(col % nzh) : 0;
   const float lyz = __ldg(lap + y) + __ldg(lap + kz);
+  float2* park = smem + N * T + threadIdx.x;          // element e of this thread at park[e * T * P]
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int i = p + P * e;
     const float k2 = __ldg(lap + i) + lyz;
-    float f = (col == 0 && i == 0) ? 0.f : scale / k2;
-    if (variant) f *= __ldg(grad + i);
-    // i f v = (-im, re) f ; stored (im, re)-swapped for the inverse transform
+    const float f = (col == 0 && i == 0) ? 0.f : scale / k2;
+    // i f v = (-im, re) f ; kept (im, re)-swapped for the inverse transform
     v[e] = make_float2(v[e].x * f, -v[e].y * f);
+    park[e * (T * P)] = v[e];
   }
   if constexpr (PL::NST > 1) __syncthreads();
   fft_line<N>(v, p, sm, tw);
   if (ok) {
-    float2* out = variant ? out_bx : out_a;
 #pragma unroll
-    for (int e = 0; e < E; ++e) out[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
+    for (int e = 0; e < E; ++e) out_a[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const float g = __ldg(grad + p + P * e);
+    const float2 a = park[e * (T * P)];
+    v[e] = make_float2(a.x * g, a.y * g);
+  }
+  if constexpr (PL::NST > 1) __syncthreads();
+  fft_line<N>(v, p, sm, tw);
+  if (ok) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) out_bx[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
   }
 }
 
@@ -105,7 +125,7 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
 // blockIdx.y, variant b % 3:  0: Bx -> Fx (in place),  1: g(w_y) A -> Fy,  2: A -> Fz (g(w_z) is applied
 // by the z pass).  in0/out0 may alias; A is read by variants 1 and 2 and written by neither.
 template <int N>
-__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P)
+__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P, cols_min_blocks<N>())
 fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
                   float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
                   int ncols, int64_t line_stride, const float2* __restrict__ tw,
