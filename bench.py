@@ -61,6 +61,21 @@ def algorithmic_bytes(n_p, ng):
     }
 
 
+def ncu_traffic(config):
+    """{kernel: dram__bytes_read.sum + dram__bytes_write.sum per launch} from profiles/ncu_traffic.csv
+    (written from the `ncu --set full` capture named in its last column; see profiles/r01_C_C4.md)."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    out = {}
+    if os.path.exists(path):
+        with open(path) as f:
+            next(f)
+            for line in f:
+                cfg, kernel, nbytes, _ = line.strip().split(",")
+                if cfg == config:
+                    out[kernel] = int(nbytes)
+    return out
+
+
 def step_bytes_unfused(n_p, ng):
     """SURVEY.md 8(d) unfused model: 96 n_p + 112 n_g bytes per PM step."""
     return 96 * n_p + 112 * ng ** 3
@@ -338,10 +353,11 @@ def main():
         kernels[name] = k
     dominant = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(args.config, {}).get(dominant)
+    traffic_table = ncu_traffic(args.config)     # per-launch DRAM bytes from the committed ncu capture
+    traffic = traffic_table.get(dominant)
+    for name, k in kernels.items():
+        if name in traffic_table:
+            k["ncu_dram_bytes"] = traffic_table[name]
     dk = kernels[dominant]
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk.get("gbs"), "peak": peak,
                 "unit": "GB/s", "frac": dk.get("frac"), "traffic": traffic, "peak_source": peak_src,
