@@ -165,3 +165,16 @@ def test_pm_step_with_arbitrary_particle_count(fpm, oracle, force_path):
     rpos = oracle.drift(pos.astype(np.float64), rmom, dr, ng)
     assert rel_l2(host(dmom), rmom) < 1e-5
     assert periodic_dist(host(dpos), rpos, ng).max() < 1e-4
+
+
+def test_full_run_C2_matches_oracle(fpm, oracle):
+    """BASELINE.json configs[1]: 128^3 / 128^3, 2LPT, 10 steps to a = 1, through the fused path."""
+    cfg = fi.CONFIGS["C2"]
+    ctx, pos, mom, rpos, rmom = _run_config(fpm, oracle, cfg, cfg.lpt_order, force_path=1)
+    dist = periodic_dist(pos, rpos, cfg.ng)
+    rms, p9999 = np.sqrt((dist ** 2).mean()), np.quantile(dist, 0.9999)
+    assert dist.max() < 1e-3, f"max {dist.max():.2e} p99.99 {p9999:.2e} rms {rms:.2e}"
+    assert rel_l2(mom, rmom) < 1e-4
+    k, pk_ref, nm = oracle.power(oracle.paint(rpos, cfg.ng), cfg.box)
+    _, pk_got, _ = oracle.power(oracle.paint(pos.astype(np.float64), cfg.ng), cfg.box)
+    assert np.max(np.abs(pk_got / pk_ref - 1)) < 1e-4
