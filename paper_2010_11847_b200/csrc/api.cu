@@ -136,12 +136,14 @@ int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, con
   Profiler* pr = &ctx->prof;
   const ParticleOrder ord = order_of(ctx, n);
   const double sc = 1.5 * ctx->cfg.omega_m;
-  // forward force meshes F_d at pos (recomputed, not stored)
-  const int rc = force_meshes(ctx, w, pos, n, false);
+  // forward force meshes F_d at pos (recomputed, not stored); interleaved when the brick walker applies
+  const bool brick = ctx->cfg.force_path == FPM_FORCE_FUSED && brick_walk_ok(n, ord, pos, v, gx);
+  const int rc = force_meshes(ctx, w, pos, n, brick);
   if (rc != FPM_OK) return rc;
   // f_d = readout(F_d, pos): direct dW/dx term
   { ProfScope sc2(pr, K_READOUT_GRAD);
-    FPM_CUDA(ctx, readout3_grad_accum(w.F[0], w.F[1], w.F[2], pos, v, (float)coef, n, ng, gx, s)); }
+    if (brick) FPM_CUDA(ctx, force_vjp_direct_brick(w.rho, pos, v, (float)coef, n, ng, gx, ord, s));
+    else FPM_CUDA(ctx, readout3_grad_accum(w.F[0], w.F[1], w.F[2], pos, v, (float)coef, n, ng, gx, s)); }
   // ... and the cotangent of the meshes: Fbar_d = paint(pos, mass = v_d)
   for (int d = 0; d < 3; ++d) {
     { ProfScope sc2(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.rho, true, ord, s)); }
@@ -153,7 +155,10 @@ int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, con
   FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.dk, w.F[0], s, pr));
   // rho = paint(pos, m): cotangent of pos = m sum_c rho_bar[c] dW/dx
   ProfScope sc2(pr, K_READOUT_GRAD);
-  FPM_CUDA(ctx, readout_grad(w.F[0], pos, nullptr, particle_mass(ctx), n, ng, gx, nullptr, s, true));
+  if (brick_walk_ok(n, ord, pos, gx, nullptr))
+    FPM_CUDA(ctx, grad_accum_brick(w.F[0], pos, particle_mass(ctx), n, ng, gx, ord, s));
+  else
+    FPM_CUDA(ctx, readout_grad(w.F[0], pos, nullptr, particle_mass(ctx), n, ng, gx, nullptr, s, true));
   return FPM_OK;
 }
 

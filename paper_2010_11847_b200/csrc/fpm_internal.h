@@ -103,6 +103,14 @@ cudaError_t readout3_grad_accum(const float* f0, const float* f1, const float* f
                                 const float* v, float coef, int64_t n, int ng, float* gx,
                                 cudaStream_t s);
 
+// Lagrangian-brick, cp.async-pipelined versions of the two gathers of the force VJP (valid when
+// brick_walk_ok: full lattice set, 16-byte aligned arrays).  f4: interleaved (F_x, F_y, F_z, -) mesh.
+bool brick_walk_ok(int64_t n, const ParticleOrder& ord, const void* a, const void* b, const void* c);
+cudaError_t force_vjp_direct_brick(const float* f4, const float* pos, const float* v, float coef,
+                                   int64_t n, int ng, float* gx, const ParticleOrder& ord, cudaStream_t s);
+cudaError_t grad_accum_brick(const float* mesh, const float* pos, float scale, int64_t n, int ng,
+                             float* gx, const ParticleOrder& ord, cudaStream_t s);
+
 // ---- particle updates (particles.cu) -----------------------------------------------------------
 cudaError_t kick(float* mom, const float* force, int64_t n3, float fac, cudaStream_t s);
 cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, cudaStream_t s);

@@ -555,6 +555,120 @@ readout3_grad_accum_kernel(const float* __restrict__ f0, const float* __restrict
   gx[2 * n + p] = fmaf(coef, az, gx[2 * n + p]);
 }
 
+// ---- generic pipelined brick walker (backward-pass gathers) ------------------------------------------
+// Same ring as rkd_pipelined_kernel, for NPL streamed planes and a per-particle functor:
+// op(vals[NPL], out[NOUT]) computes NOUT results that are stored to the planes dst[0..NOUT-1].
+template <int NPL>
+struct Planes { const float* src[NPL]; };
+template <int NOUT>
+struct OutPlanes { float* dst[NOUT]; };
+
+template <int STAGES, int NPL, int NOUT, class OP>
+__global__ void __launch_bounds__(kThreads, 4)
+brick_gather_kernel(Planes<NPL> in, OutPlanes<NOUT> out, BrickMap bm, OP op) {
+  constexpr int DIST = STAGES - 1, NCP = NPL * 8, CPL = (NCP + 31) / 32;
+  __shared__ __align__(16) float ring[STAGES][NPL][kThreads];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  int qx0, qy0, qz0;
+  bm.origin(blockIdx.x >> 1, qx0, qy0, qz0);
+  const int64_t plane = (int64_t)bm.np * bm.np;
+  const int64_t row0 = ((int64_t)qx0 * bm.np + (qy0 + (BY / 2) * (blockIdx.x & 1) + warp)) * bm.np + qz0;
+  auto issue = [&](int b) {
+    const int st = b % STAGES;
+#pragma unroll
+    for (int i = 0; i < CPL; ++i) {
+      const int t = lane + 32 * i, a = t >> 3, c = t & 7;
+      if (NCP % 32 != 0 && t >= NCP) break;
+      cp_async16(&ring[st][a][warp * 32 + 4 * c], in.src[a] + row0 + (int64_t)b * plane + 4 * c);
+    }
+  };
+#pragma unroll
+  for (int b = 0; b < DIST; ++b) { if (b < BX) issue(b); cp_async_commit(); }
+#pragma unroll 1
+  for (int b = 0; b < BX; ++b) {
+    if (b + DIST < BX) issue(b + DIST);
+    cp_async_commit();
+    cp_async_wait<DIST>();
+    __syncwarp();
+    const int st = b % STAGES;
+    float vals[NPL], res[NOUT];
+#pragma unroll
+    for (int a = 0; a < NPL; ++a) vals[a] = ring[st][a][tid];
+    op(vals, res);
+    const int64_t p = row0 + lane + (int64_t)b * plane;
+#pragma unroll
+    for (int a = 0; a < NOUT; ++a) __stcs(out.dst[a] + p, res[a]);
+    __syncwarp();
+  }
+}
+
+// planes: x y z | v0 v1 v2 | gx gy gz ; result: g + coef * sum_d v_d sum_c F_d[c] dW/dx  (interleaved F)
+struct ForceVjpDirectOp {
+  const float4* mesh;
+  unsigned g;
+  float coef;
+  __device__ __forceinline__ void operator()(const float (&v)[9], float (&r)[3]) const {
+    const Cic c = cic_of(v[0], v[1], v[2], (int)g - 1);
+    const float wx[2] = {1.f - c.t[0], c.t[0]}, wy[2] = {1.f - c.t[1], c.t[1]}, wz[2] = {1.f - c.t[2], c.t[2]};
+    const float sg[2] = {-1.f, 1.f};
+    const unsigned ix[2] = {(unsigned)c.i0[0] * g, (unsigned)c.i1[0] * g};
+    const unsigned iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]}, iz[2] = {(unsigned)c.i0[2], (unsigned)c.i1[2]};
+    float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        const unsigned row = (ix[a] + iy[b]) * g;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const float4 F = __ldg(mesh + (row + iz[e]));
+          const float f = v[3] * F.x + v[4] * F.y + v[5] * F.z;
+          ax = fmaf(f, sg[a] * wy[b] * wz[e], ax);
+          ay = fmaf(f, wx[a] * sg[b] * wz[e], ay);
+          az = fmaf(f, wx[a] * wy[b] * sg[e], az);
+        }
+      }
+    r[0] = fmaf(coef, ax, v[6]);
+    r[1] = fmaf(coef, ay, v[7]);
+    r[2] = fmaf(coef, az, v[8]);
+  }
+};
+
+// planes: x y z | gx gy gz ; result: g + scale * sum_c mesh[c] dW/dx
+struct GradAccumOp {
+  const float* mesh;
+  unsigned g;
+  float scale;
+  __device__ __forceinline__ void operator()(const float (&v)[6], float (&r)[3]) const {
+    const Cic c = cic_of(v[0], v[1], v[2], (int)g - 1);
+    const float wx[2] = {1.f - c.t[0], c.t[0]}, wy[2] = {1.f - c.t[1], c.t[1]}, wz[2] = {1.f - c.t[2], c.t[2]};
+    const float sg[2] = {-1.f, 1.f};
+    const unsigned ix[2] = {(unsigned)c.i0[0] * g, (unsigned)c.i1[0] * g};
+    const unsigned iy[2] = {(unsigned)c.i0[1], (unsigned)c.i1[1]}, iz[2] = {(unsigned)c.i0[2], (unsigned)c.i1[2]};
+    float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        const unsigned row = (ix[a] + iy[b]) * g;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const float f = __ldg(mesh + (row + iz[e]));
+          ax = fmaf(f, sg[a] * wy[b] * wz[e], ax);
+          ay = fmaf(f, wx[a] * sg[b] * wz[e], ay);
+          az = fmaf(f, wx[a] * wy[b] * sg[e], az);
+        }
+      }
+    r[0] = fmaf(scale, ax, v[3]);
+    r[1] = fmaf(scale, ay, v[4]);
+    r[2] = fmaf(scale, az, v[5]);
+  }
+};
+
+inline bool aligned16(const void* a, const void* b = nullptr, const void* c = nullptr) {
+  return ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(b) | reinterpret_cast<uintptr_t>(c)) & 15) == 0;
+}
+
 inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kThreads - 1) / kThreads); }
 
 inline BrickMap brick_map(int np) { return BrickMap{np, np / BZ, np / BY}; }
@@ -650,6 +764,30 @@ cudaError_t readout3_grad_accum(const float* f0, const float* f1, const float* f
                                 cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   readout3_grad_accum_kernel<<<blocks_for(n), kThreads, 0, s>>>(f0, f1, f2, pos, v, coef, n, ng, gx);
+  return cudaGetLastError();
+}
+
+bool brick_walk_ok(int64_t n, const ParticleOrder& ord, const void* a, const void* b, const void* c) {
+  return brick_ok(n, ord.np) && aligned16(a, b, c);
+}
+
+cudaError_t force_vjp_direct_brick(const float* f4, const float* pos, const float* v, float coef,
+                                   int64_t n, int ng, float* gx, const ParticleOrder& ord, cudaStream_t s) {
+  if (!brick_walk_ok(n, ord, pos, v, gx)) return cudaErrorInvalidValue;
+  Planes<9> in{{pos, pos + n, pos + 2 * n, v, v + n, v + 2 * n, gx, gx + n, gx + 2 * n}};
+  OutPlanes<3> out{{gx, gx + n, gx + 2 * n}};
+  ForceVjpDirectOp op{reinterpret_cast<const float4*>(f4), (unsigned)ng, coef};
+  brick_gather_kernel<3, 9, 3, ForceVjpDirectOp><<<(unsigned)(2 * (n / kBrick)), kThreads, 0, s>>>(in, out, brick_map(ord.np), op);
+  return cudaGetLastError();
+}
+
+cudaError_t grad_accum_brick(const float* mesh, const float* pos, float scale, int64_t n, int ng,
+                             float* gx, const ParticleOrder& ord, cudaStream_t s) {
+  if (!brick_walk_ok(n, ord, pos, gx, nullptr)) return cudaErrorInvalidValue;
+  Planes<6> in{{pos, pos + n, pos + 2 * n, gx, gx + n, gx + 2 * n}};
+  OutPlanes<3> out{{gx, gx + n, gx + 2 * n}};
+  GradAccumOp op{mesh, (unsigned)ng, scale};
+  brick_gather_kernel<3, 6, 3, GradAccumOp><<<(unsigned)(2 * (n / kBrick)), kThreads, 0, s>>>(in, out, brick_map(ord.np), op);
   return cudaGetLastError();
 }
 
