@@ -40,6 +40,16 @@ __device__ __forceinline__ float fast_floor(float x, int& i) {
   return r;
 }
 __device__ __forceinline__ int fast_round_to_int(float x) { return __float_as_int(x + kMagic) - kMagicBits; }
+// round(a * b) with one rounding: the product is formed inside the FMA that adds the magic constant
+__device__ __forceinline__ int fast_round_mul_to_int(float a, float b) {
+  return __float_as_int(fmaf(a, b, kMagic)) - kMagicBits;
+}
+// CIC split without compare/select: i = rint(x - 1/2), t = x - i.  Equal to (floor(x), x - floor(x)) unless
+// x is an integer k, where it may give (k - 1, 1) instead of (k, 0): the same deposit (weight 1 on cell k).
+__device__ __forceinline__ float cic_split(float x, int& i) {
+  const float r = fast_rint(x - 0.5f, i);
+  return x - r;
+}
 
 __device__ __forceinline__ Cic cic_of(float x, float y, float z, int mask) {
   Cic c;
@@ -212,8 +222,7 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
     int ix, iy, iz;
-    const float fx = fast_floor(x[k], ix), fy = fast_floor(y[k], iy), fz = fast_floor(z[k], iz);
-    const float tx = x[k] - fx, ty = y[k] - fy, tz = z[k] - fz;
+    const float tx = cic_split(x[k], ix), ty = cic_split(y[k], iy), tz = cic_split(z[k], iz);
     const unsigned rx = (ix - ox) & mask, ry = (iy - oy) & mask, rz = (iz - oz) & mask;
     const float mk = HAS_MASS ? m[k] : mass_const;
     if (rx < WX - 1 && ry < WY - 1 && rz < WZ - 1) {
@@ -224,14 +233,14 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
       const int base = (rx * WY + ry) * WZ + rz;
       if (FIXED) {
         int* c = win_i + base;
-        atomicAdd(c, fast_round_to_int(w00 * wz0));
-        atomicAdd(c + 1, fast_round_to_int(w00 * wz1));
-        atomicAdd(c + WZ, fast_round_to_int(w01 * wz0));
-        atomicAdd(c + WZ + 1, fast_round_to_int(w01 * wz1));
-        atomicAdd(c + WY * WZ, fast_round_to_int(w10 * wz0));
-        atomicAdd(c + WY * WZ + 1, fast_round_to_int(w10 * wz1));
-        atomicAdd(c + WY * WZ + WZ, fast_round_to_int(w11 * wz0));
-        atomicAdd(c + WY * WZ + WZ + 1, fast_round_to_int(w11 * wz1));
+        atomicAdd(c, fast_round_mul_to_int(w00, wz0));
+        atomicAdd(c + 1, fast_round_mul_to_int(w00, wz1));
+        atomicAdd(c + WZ, fast_round_mul_to_int(w01, wz0));
+        atomicAdd(c + WZ + 1, fast_round_mul_to_int(w01, wz1));
+        atomicAdd(c + WY * WZ, fast_round_mul_to_int(w10, wz0));
+        atomicAdd(c + WY * WZ + 1, fast_round_mul_to_int(w10, wz1));
+        atomicAdd(c + WY * WZ + WZ, fast_round_mul_to_int(w11, wz0));
+        atomicAdd(c + WY * WZ + WZ + 1, fast_round_mul_to_int(w11, wz1));
       } else {
         float* c = win_f + base;
         atomicAdd(c, w00 * wz0);
