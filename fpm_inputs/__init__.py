@@ -13,8 +13,10 @@ from .fields import (
     counter_uniform,
     eh_nowiggle_transfer,
     eh_sound_horizon_and_alpha,
+    inverse_prior_power,
     linear_field,
     linear_power,
+    noise_field,
     power_amplitude,
     random_particles,
     sigma_r,
@@ -24,6 +26,6 @@ from .fields import (
 __all__ = [
     "CONFIGS", "COSMO", "Config",
     "counter_normal", "counter_uniform", "eh_nowiggle_transfer",
-    "eh_sound_horizon_and_alpha", "linear_field", "linear_power",
+    "eh_sound_horizon_and_alpha", "inverse_prior_power", "linear_field", "linear_power", "noise_field",
     "power_amplitude", "random_particles", "sigma_r", "weight_field",
 ]

@@ -133,6 +133,26 @@ def linear_field(np_side, box, seed, cosmo=COSMO):
     return np.ascontiguousarray(out, dtype=np.float32)
 
 
+def inverse_prior_power(np_side, box, cosmo=COSMO):
+    """Table 1/<|s_k|^2> of the Gaussian prior of N1 (Eq. 12; Listing 7.1 "r2c(var)^2/power")
+    on the half-complex layout [n][n][n/2+1], float32: for the field of linear_field(), the unnormalised
+    DFT has <|s_k|^2> = n^3 P(k) / V_cell.  The k = 0 entry is 0 (the mean is not constrained)."""
+    n = int(np_side)
+    kf = 2.0 * math.pi / box
+    vcell = (box / n) ** 3
+    fx = np.fft.fftfreq(n, 1.0 / n)
+    fz = np.arange(n // 2 + 1, dtype=np.float64)
+    k2 = fx[:, None, None] ** 2 + fx[None, :, None] ** 2 + fz[None, None, :] ** 2
+    var = n ** 3 * linear_power(kf * np.sqrt(k2), cosmo) / vcell
+    out = np.where(var > 0, 1.0 / np.where(var > 0, var, 1.0), 0.0)
+    return np.ascontiguousarray(out, dtype=np.float32)
+
+
+def noise_field(ng, sigma, seed=202):
+    """Uncorrelated Gaussian data noise of standard deviation sigma on the Ng mesh."""
+    return (sigma * _normal_grid(seed, int(ng), dtype=np.float64)).astype(np.float32)
+
+
 def weight_field(ng, seed=101):
     """Seeded N(0,1) weight field on the Ng mesh (objective of C4's backward pass, R12)."""
     return _normal_grid(seed, int(ng), dtype=np.float32)

@@ -247,3 +247,25 @@ def lpt_init_vjp(delta_lin, ng, omega_m, a0, order, gx, gp):
     _load().orc_lpt_init_vjp(_p(d), ctypes.c_int(np_side), ctypes.c_int(ng), ctypes.c_double(omega_m),
                              ctypes.c_double(a0), ctypes.c_int(order), _p(gx), _p(gp), _p(out))
     return out
+
+
+def recon_loss_grad(s, ng, omega_m, a0, order, stages, data, sigma, inv_power, mode=KERNEL_PAPER,
+                    factor_mode=FACTORS_FASTPM):
+    """N1 (Eq. 12): (chi2 term, prior term), gradient w.r.t. the real linear field s [np^3]."""
+    s, data, ip = _f64(s), _f64(data), _f64(inv_power)
+    np_side = s.shape[0]
+    st = _f64(stages)
+    grad, loss2 = np.zeros(s.shape), np.zeros(2)
+    _load().orc_recon_loss_grad(_p(s), ctypes.c_int(np_side), ctypes.c_int(ng), ctypes.c_double(omega_m),
+                                ctypes.c_int(mode), ctypes.c_int(factor_mode), ctypes.c_double(a0),
+                                ctypes.c_int(order), _p(st), ctypes.c_int(len(st) - 1), _p(data),
+                                ctypes.c_double(sigma), _p(ip), _p(grad), _p(loss2))
+    return (float(loss2[0]), float(loss2[1])), grad
+
+
+def adam_step(x, g, m, v, lr, t, b1=0.9, b2=0.999, eps=1e-8):
+    """One Adam update (in float64); returns new (x, m, v)."""
+    x, m, v, g = _f64(x).copy(), _f64(m).copy(), _f64(v).copy(), _f64(g)
+    _load().orc_adam_step(_p(x), _p(g), _p(m), _p(v), ctypes.c_int64(x.size), ctypes.c_double(lr),
+                          ctypes.c_double(b1), ctypes.c_double(b2), ctypes.c_double(eps), ctypes.c_int(t))
+    return x, m, v

@@ -650,6 +650,72 @@ void lpt_init_vjp_impl(const double* delta_lin, int np, int ng, double om, doubl
 }
 
 // ------------------------------------------------------------------------------------------
+// N1  MAP reconstruction of the initial field (Eq. 12; Listing 7.1):
+//   -log p = sum_c (delta_e - delta_m)^2 / (2 sigma^2) + 1/2 s^dagger S^-1 s,   delta_m = F(s).
+// Readings: F(s) = paint(nbody(lpt_init(s))) with mean density 1, so
+// delta_e - delta_m = data - rho_m when data is also a mean-1 density; the prior is diagonal in k:
+// 1/2 sum over the FULL k-space of |s_k|^2 inv_power[k], s_k the unnormalised DFT of s, inv_power the
+// caller's table 1/<|s_k|^2> on the half-complex layout (Listing 7.1: "prior = sum(r2c(var)^2/power)");
+// the listing's chisq has no 1/2 -- Eq. 12 is followed.  Gradient of the prior w.r.t. the real field:
+// n^3 c2r(inv_power s_k).  Optimiser: Adam (Listing 7.1), textbook update with bias correction.
+// ------------------------------------------------------------------------------------------
+void recon_loss_grad_impl(const double* s, int np, int ng, double om, int mode, int factor_mode,
+                          double a0, int order, const double* stages, int n_steps, const double* data,
+                          double sigma, const double* inv_power, double* grad, double* loss2) {
+  const int64_t n = (int64_t)np * np * np, g3 = (int64_t)ng * ng * ng, nzh = np / 2 + 1,
+                nk = (int64_t)np * np * nzh;
+  const double B = (double)ng / np, mass = B * B * B;
+  // forward model
+  std::vector<double> pos(3 * n), mom(3 * n), traj((size_t)(n_steps + 1) * 3 * n), rho(g3);
+  lpt_init_impl(s, np, ng, om, a0, order, pos.data(), mom.data());
+  nbody_impl(pos.data(), mom.data(), n, ng, np, om, mode, factor_mode, stages, n_steps, traj.data());
+  paint_impl(pos.data(), nullptr, mass, n, ng, rho.data());
+  // likelihood term and its cotangent on the mesh
+  std::vector<double> gbar(g3);
+  double chi2 = 0.0;
+  for (int64_t i = 0; i < g3; ++i) {
+    const double r = rho[i] - data[i];
+    chi2 += r * r;
+    gbar[i] = r / (sigma * sigma);
+  }
+  loss2[0] = 0.5 * chi2 / (sigma * sigma);
+  // reverse: paint -> nbody -> lpt_init
+  std::vector<double> gx(3 * n), gp(3 * n, 0.0);
+  readout_grad_impl(gbar.data(), pos.data(), n, ng, gx.data());
+  for (int64_t i = 0; i < 3 * n; ++i) gx[i] *= mass;
+  nbody_vjp_impl(traj.data(), n, ng, np, om, mode, factor_mode, stages, n_steps, gx.data(), gp.data());
+  lpt_init_vjp_impl(s, np, ng, om, a0, order, gx.data(), gp.data(), grad);
+  // prior term
+  std::vector<double> sk(2 * nk), gk(2 * nk), gprior(n);
+  r2c_impl(s, np, sk.data(), false);
+  double prior = 0.0;
+  for (int64_t x = 0; x < np; ++x)
+    for (int64_t y = 0; y < np; ++y)
+      for (int64_t z = 0; z < nzh; ++z) {
+        const int64_t i = (x * np + y) * nzh + z;
+        const double wt = (z == 0 || 2 * z == np) ? 1.0 : 2.0;      // Hermitian half implied
+        prior += wt * inv_power[i] * (sk[2 * i] * sk[2 * i] + sk[2 * i + 1] * sk[2 * i + 1]);
+        gk[2 * i] = inv_power[i] * sk[2 * i] * (double)n;
+        gk[2 * i + 1] = inv_power[i] * sk[2 * i + 1] * (double)n;
+      }
+  loss2[1] = 0.5 * prior;
+  c2r_impl(gk.data(), np, gprior.data(), false);
+  for (int64_t i = 0; i < n; ++i) grad[i] += gprior[i];
+}
+
+// Adam (Kingma & Ba), step t >= 1:  m = b1 m + (1-b1) g ; v = b2 v + (1-b2) g^2 ;
+// x -= lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps)
+void adam_step_impl(double* x, const double* g, double* m, double* v, int64_t n, double lr, double b1,
+                    double b2, double eps, int t) {
+  const double c1 = 1.0 - std::pow(b1, t), c2 = 1.0 - std::pow(b2, t);
+  for (int64_t i = 0; i < n; ++i) {
+    m[i] = b1 * m[i] + (1.0 - b1) * g[i];
+    v[i] = b2 * v[i] + (1.0 - b2) * g[i] * g[i];
+    x[i] -= lr * (m[i] / c1) / (std::sqrt(v[i] / c2) + eps);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // R13  Binned power spectrum: |deltahat|^2 V / n_g^2, bins of width k_f centred on integers,
 // half-space weights (2 for 0 < nz < ng/2, else 1); cross spectrum for Eq. 10-11.
 // ------------------------------------------------------------------------------------------
@@ -810,6 +876,19 @@ void orc_nbody_vjp(const double* traj, int64_t n, int ng, int np, double om, int
 void orc_lpt_init_vjp(const double* delta_lin, int np, int ng, double om, double a0, int order,
                       const double* gx, const double* gp, double* gdelta) {
   lpt_init_vjp_impl(delta_lin, np, ng, om, a0, order, gx, gp, gdelta);
+}
+
+
+// ---- N1 reconstruction ----------------------------------------------------------------------------
+void orc_recon_loss_grad(const double* s, int np, int ng, double om, int mode, int factor_mode, double a0,
+                         int order, const double* stages, int n_steps, const double* data, double sigma,
+                         const double* inv_power, double* grad, double* loss2) {
+  recon_loss_grad_impl(s, np, ng, om, mode, factor_mode, a0, order, stages, n_steps, data, sigma,
+                       inv_power, grad, loss2);
+}
+void orc_adam_step(double* x, const double* g, double* m, double* v, int64_t n, double lr, double b1,
+                   double b2, double eps, int t) {
+  adam_step_impl(x, g, m, v, n, lr, b1, b2, eps, t);
 }
 
 }  // extern "C"
