@@ -212,6 +212,29 @@ int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n
 int fpm_lpt_init_vjp(fpm_ctx* ctx, const float* delta_lin, double a0, int order,
                      const float* grad_pos, const float* grad_mom, float* grad_delta);
 
+/* ---- MAP reconstruction of the linear field (Eq. 12, Listing 7.1) -- */
+
+/* Bytes of caller-owned DEVICE scratch fpm_recon_loss_grad needs for a forward model of n_steps steps:
+ * pos, mom, their cotangents and the trajectory, (n_steps + 5) * 3 * np^3 floats (0 on invalid input). */
+size_t fpm_recon_scratch_bytes(const fpm_config* cfg, int n_steps);
+
+/* Negative log-posterior of the linear field s and its gradient (Eq. 12):
+ *   loss = 1/2 sum_c ((rho_m[c] - data[c]) / sigma)^2 + 1/2 sum_k |s_k|^2 inv_power[k],
+ *   rho_m = paint(nbody(lpt_init(s, a_stages[0], lpt_order), a_stages)), mean density 1,
+ *   s_k the unnormalised DFT of s, the k sum over the full k-space.
+ * s [np^3] DEVICE; data [ng^3] DEVICE (a mean-1 density); inv_power [np*np*(np/2+1)] DEVICE real table
+ * 1/<|s_k|^2> (0 where a mode is unconstrained); a_stages HOST [n_steps+1]; scratch DEVICE, 16-byte
+ * aligned; grad [np^3] DEVICE = d loss / d s (overwritten); loss HOST double[2] = {likelihood term,
+ * prior term}.  Needs the workspace; synchronises the stream before returning (the loss is read back). */
+int fpm_recon_loss_grad(fpm_ctx* ctx, const float* s, const float* data, double sigma,
+                        const float* inv_power, const double* a_stages, int n_steps, int lpt_order,
+                        void* scratch, size_t scratch_bytes, float* grad, double* loss);
+
+/* One Adam update (Listing 7.1 "AdamOptimizer"), step t >= 1, all arrays DEVICE [n]:
+ * m = b1 m + (1-b1) g; v = b2 v + (1-b2) g^2; x -= lr (m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps). */
+int fpm_adam_step(fpm_ctx* ctx, float* x, const float* grad, float* m, float* v, int64_t n, double lr,
+                  double beta1, double beta2, double eps, int t);
+
 /* ---- measurement hooks -------------------------------------------------------------------- */
 /* Per-kernel CUDA-event timing on the context's stream (off by default).  fpm_profile_read
  * synchronises the recorded events; kernel_id runs over 0 .. until FPM_EINVAL is returned.

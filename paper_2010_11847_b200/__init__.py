@@ -73,6 +73,10 @@ def _load():
         "fpm_force_vjp": (i32, [vp, vp, i64, vp, dbl, vp]),
         "fpm_nbody_vjp": (i32, [vp, vp, ctypes.POINTER(dbl), i32, vp, vp]),
         "fpm_lpt_init_vjp": (i32, [vp, vp, dbl, i32, vp, vp, vp]),
+        "fpm_recon_scratch_bytes": (ctypes.c_size_t, [ctypes.POINTER(_Config), i32]),
+        "fpm_recon_loss_grad": (i32, [vp, vp, vp, dbl, vp, ctypes.POINTER(dbl), i32, i32, vp, ctypes.c_size_t, vp,
+                                      ctypes.POINTER(dbl)]),
+        "fpm_adam_step": (i32, [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, i32]),
         "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
         "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
     }
@@ -333,3 +337,24 @@ class FPM:
         self._check(_lib.fpm_lpt_init_vjp(self._h, _dev(delta_lin), a0, order, _dev(grad_pos),
                                           _dev(grad_mom), _dev(out)))
         return out
+
+    # ---- MAP reconstruction (Eq. 12, Listing 7.1) -------------------
+    def recon_loss_grad(self, s, data, sigma, inv_power, stages, lpt_order=2, scratch=None):
+        """((likelihood term, prior term), gradient [np^3]) of the negative log-posterior of s."""
+        n_steps = len(stages) - 1
+        need = _lib.fpm_recon_scratch_bytes(ctypes.byref(self._cfg), n_steps)
+        if scratch is None or scratch.numel() * scratch.element_size() < need:
+            scratch = torch.empty(need // 4, dtype=torch.float32, device=self.device)
+            self._recon_scratch = scratch
+        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+        grad = self._empty(self.np_side, self.np_side, self.np_side)
+        loss = (ctypes.c_double * 2)()
+        self._check(_lib.fpm_recon_loss_grad(self._h, _dev(s), _dev(data), float(sigma), _dev(inv_power), st,
+                                             n_steps, int(lpt_order), ctypes.c_void_p(scratch.data_ptr()),
+                                             scratch.numel() * scratch.element_size(), _dev(grad), loss))
+        return (loss[0], loss[1]), grad
+
+    def adam_step(self, x, grad, m, v, lr, t, beta1=0.9, beta2=0.999, eps=1e-8):
+        self._check(_lib.fpm_adam_step(self._h, _dev(x), _dev(grad), _dev(m), _dev(v), x.numel(), lr, beta1,
+                                       beta2, eps, int(t)))
+        return x

@@ -186,6 +186,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
   if (e == cudaSuccess) e = fft_tables_create(cfg->np, &ctx->fft_p);
   if (e == cudaSuccess) e = kernel_tables_create(cfg->ng, cfg->kernel_mode, &ctx->kt_g);
   if (e == cudaSuccess) e = kernel_tables_create(cfg->np, FPM_KERNEL_NAIVE, &ctx->kt_p);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_acc, 2 * sizeof(double));
   if (e != cudaSuccess) {
     fpm_destroy(ctx);
     return FPM_ECUDA;
@@ -197,6 +198,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
 int fpm_destroy(fpm_ctx* ctx) {
   if (!ctx) return FPM_EINVAL;
   ctx->prof.destroy();
+  if (ctx->d_acc) cudaFree(ctx->d_acc);
   fft_tables_destroy(&ctx->fft_g);
   fft_tables_destroy(&ctx->fft_p);
   kernel_tables_destroy(&ctx->kt_g);
@@ -568,6 +570,76 @@ int fpm_lpt_init_vjp(fpm_ctx* ctx, const float* delta_lin, double a0, int order,
     }
   }
   FPM_CUDA(ctx, fft_c2r(ctx->fft_p, acck, grad_delta, s, pr));
+  return FPM_OK;
+}
+
+size_t fpm_recon_scratch_bytes(const fpm_config* cfg, int n_steps) {
+  if (!config_ok(cfg) || n_steps < 0) return 0;
+  const size_t n = (size_t)cfg->np * cfg->np * cfg->np;
+  return sizeof(float) * 3 * n * ((size_t)n_steps + 5);
+}
+
+int fpm_recon_loss_grad(fpm_ctx* ctx, const float* s_lin, const float* data, double sigma,
+                        const float* inv_power, const double* a_stages, int n_steps, int lpt_order,
+                        void* scratch, size_t scratch_bytes, float* grad, double* loss) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, s_lin && data && inv_power && a_stages && scratch && grad && loss && n_steps >= 0,
+              "fpm_recon_loss_grad: bad arguments");
+  FPM_REQUIRE(ctx, sigma > 0.0, "fpm_recon_loss_grad: sigma must be positive");
+  FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(scratch) & 15) == 0, "fpm_recon_loss_grad: scratch must be 16-byte aligned");
+  if (scratch_bytes < fpm_recon_scratch_bytes(&ctx->cfg, n_steps))
+    return fail(ctx, FPM_ENOMEM, "fpm_recon_loss_grad: scratch too small (fpm_recon_scratch_bytes)");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  cudaStream_t st = ctx->stream;
+  Profiler* pr = &ctx->prof;
+  const int np = ctx->cfg.np, ng = ctx->cfg.ng;
+  const int64_t n = (int64_t)np * np * np, g3 = (int64_t)ng * ng * ng;
+  float* pos = static_cast<float*>(scratch);
+  float *mom = pos + 3 * n, *gx = mom + 3 * n, *gp = gx + 3 * n, *traj = gp + 3 * n;
+  FPM_CUDA(ctx, cudaMemsetAsync(ctx->d_acc, 0, 2 * sizeof(double), st));
+  // forward model F(s) (Listing 7.1 "model = FLOWPM(var, ...)")
+  int rc = fpm_lpt_init(ctx, s_lin, a_stages[0], lpt_order, pos, mom);
+  if (rc != FPM_OK) return rc;
+  rc = fpm_nbody(ctx, pos, mom, a_stages, n_steps, traj);
+  if (rc != FPM_OK) return rc;
+  { ProfScope sc(pr, K_PAINT);
+    FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), st)); }
+  // likelihood term and its cotangent on the mesh
+  ctx->prof.launches += 1;
+  FPM_CUDA(ctx, recon_residual(w.rho, data, (float)(1.0 / (sigma * sigma)), g3, w.F[0], ctx->d_acc, st));
+  // reverse: paint -> run -> initial conditions
+  { ProfScope sc(pr, K_READOUT_GRAD);
+    FPM_CUDA(ctx, readout_grad(w.F[0], pos, nullptr, particle_mass(ctx), n, ng, gx, nullptr, st)); }
+  FPM_CUDA(ctx, cudaMemsetAsync(gp, 0, sizeof(float) * 3 * n, st));
+  rc = fpm_nbody_vjp(ctx, traj, a_stages, n_steps, gx, gp);
+  if (rc != FPM_OK) return rc;
+  rc = fpm_lpt_init_vjp(ctx, s_lin, a_stages[0], lpt_order, gx, gp, grad);
+  if (rc != FPM_OK) return rc;
+  // prior term (Listing 7.1 "prior = sum(r2c(var)^2 / power)") and its gradient n^3 c2r(inv_power s_k)
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_p, s_lin, w.dk, st, pr));
+  ctx->prof.launches += 1;
+  FPM_CUDA(ctx, recon_prior(w.dk, inv_power, np, w.fk[0], ctx->d_acc + 1, st));
+  FPM_CUDA(ctx, fft_c2r(ctx->fft_p, w.fk[0], w.F[0], st, pr));
+  ctx->prof.launches += 1;
+  FPM_CUDA(ctx, axpy(grad, w.F[0], 1.f, n, st));
+  double acc[2];
+  FPM_CUDA(ctx, cudaMemcpyAsync(acc, ctx->d_acc, sizeof acc, cudaMemcpyDeviceToHost, st));
+  FPM_CUDA(ctx, cudaStreamSynchronize(st));
+  loss[0] = 0.5 * acc[0] / (sigma * sigma);
+  loss[1] = 0.5 * acc[1];
+  return FPM_OK;
+}
+
+int fpm_adam_step(fpm_ctx* ctx, float* x, const float* grad, float* m, float* v, int64_t n, double lr,
+                  double beta1, double beta2, double eps, int t) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, n >= 0 && ((x && grad && m && v) || n == 0), "fpm_adam_step: bad arguments");
+  FPM_REQUIRE(ctx, t >= 1 && beta1 >= 0.0 && beta1 < 1.0 && beta2 >= 0.0 && beta2 < 1.0, "fpm_adam_step: bad hyper-parameters");
+  if (n == 0) return FPM_OK;
+  const double c1 = 1.0 - std::pow(beta1, t), c2 = 1.0 - std::pow(beta2, t);
+  ctx->prof.launches += 1;
+  FPM_CUDA(ctx, adam_update(x, grad, m, v, n, lr, beta1, beta2, eps, 1.0 / c1, 1.0 / c2, ctx->stream));
   return FPM_OK;
 }
 

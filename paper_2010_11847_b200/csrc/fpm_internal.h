@@ -143,6 +143,14 @@ cudaError_t lpt_wrap(float* pos, int64_t n3, int ng, cudaStream_t s);
 cudaError_t lpt_source(float* s, const float* a, const float* b, const float* c, int64_t n, int mode,
                        cudaStream_t st);
 
+// ---- MAP reconstruction element-wise kernels (recon.cu) ----------------------
+cudaError_t recon_residual(const float* rho, const float* data, float inv_s2, int64_t n, float* gbar,
+                           double* acc, cudaStream_t s);
+cudaError_t recon_prior(const float2* sk, const float* inv_power, int n, float2* gk, double* acc,
+                        cudaStream_t s);
+cudaError_t adam_update(float* x, const float* g, float* m, float* v, int64_t n, double lr, double b1,
+                        double b2, double eps, double inv_c1, double inv_c2, cudaStream_t s);
+
 // ---- background cosmology on the host, float64 (cosmology.cpp) ---------------------------------
 struct GrowthOut { double D1, f1, D2, f2, E, Gf, gf; };
 GrowthOut growth(double omega_m, double a);
@@ -158,6 +166,7 @@ struct fpm_ctx {
   fpm::KernelTables kt_g, kt_p;     // transfer-function tables on ng; spectral tables on np
   void* ws = nullptr;
   size_t ws_bytes = 0;
+  double* d_acc = nullptr;          // two float64 accumulators (loss terms of fpm_recon_loss_grad)
   bool sticky = false;
   std::string err;
   fpm::Profiler prof;
