@@ -228,6 +228,36 @@ def side_measurements(args, ctx, cfg, pos, mom, factors, device):
     out["backward_step"] = {"ms": ms_bwd, "call": "fpm_force_vjp (one backward force evaluation of fpm_nbody_vjp)",
                             "steps_per_s": 1e3 / ms_bwd}
     del gx, v
+    torch.cuda.empty_cache()
+    # (iii) SURVEY.md 8(f) N1: one MAP-reconstruction iteration (loss + gradient through a 5-step 128^3 PM
+    # forward model in a 400 Mpc/h box + Adam update), the configuration of PAPER.md:490-502.
+    import paper_2010_11847_b200 as fpm
+    n_r, box_r = 128, 400.0
+    rctx = fpm.FPM(n_r, n_r, omega_m=fi.COSMO["omega_m"], box=box_r, device=device, force_path=fpm.FORCE_FUSED)
+    stages = [0.1 + j * 0.9 / 5 for j in range(6)]
+    truth = torch.from_numpy(fi.linear_field(n_r, box_r, 6)).to(device)
+    p0, m0 = rctx.lpt_init(truth, stages[0], 2)
+    rctx.nbody(p0, m0, stages)
+    data = rctx.paint(p0) + torch.from_numpy(fi.noise_field(n_r, 1.0)).to(device)   # synthetic "observation"
+    ipow = torch.from_numpy(fi.inverse_prior_power(n_r, box_r)).to(device)
+    s = torch.zeros(n_r, n_r, n_r, device=device)
+    am, av = torch.zeros_like(s), torch.zeros_like(s)
+    state = {"t": 0, "loss": None}
+
+    def iteration():
+        state["t"] += 1
+        loss, g = rctx.recon_loss_grad(s, data, 1.0, ipow, stages, 2)
+        rctx.adam_step(s, g, am, av, 0.01, state["t"])
+        state["loss"] = loss[0] + loss[1]
+
+    iteration()
+    first = state["loss"]
+    ms_it = timed(iteration, 10)
+    out["recon_iteration"] = {"ms": ms_it, "config": "5-step 128^3 PM forward model, 400 Mpc/h box, 2LPT ICs, loss + "
+                              "gradient (fpm_recon_loss_grad) + Adam (fpm_adam_step)", "loss_first": first,
+                              "loss_after_11_iterations": state["loss"],
+                              "paper_context": "1.1 s/iteration on one V100, 4.6 s on 128 Haswell cores (PAPER.md:502)"}
+    rctx.close()
     return out
 
 
