@@ -124,9 +124,11 @@ cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t
   return launch_z_c2r<N>(t, cplx, real, nullptr, s, prof);
 }
 
-// Fused force meshes (DESIGN.md section 5): r2c z, y forward, x round trip with the transfer
-// function (2 variants), 3 inverse y passes in one launch, 3 c2r z passes (g(w_z) fused into the
-// third).  wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.
+// Fused force meshes (DESIGN.md section 5.2): r2c z, y forward, x round trip with the transfer
+// function (one forward, two inverse transforms per column), 3 inverse y passes in one launch, then
+// either 3 planar c2r z passes into F[0..2] or, when F4 is given, one launch writing the interleaved
+// (F_x, F_y, F_z, 0) mesh (g(w_z) fused into the z pass of the third component either way).
+// wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.
 template <int N>
 cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                              float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,

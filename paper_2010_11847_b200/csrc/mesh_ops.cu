@@ -5,8 +5,10 @@
 // sm_100a design:
 //   * Particles of a run are stored in Lagrangian (lattice) order and move a few cells at most, so a
 //     brick of 8 x 16 x 32 lattice neighbours stays a compact Eulerian cloud.  One CTA owns one
-//     brick.  Readout: the brick's gathers hit the same few mesh rows, which therefore stay in that
-//     SM's L1; bricks are scheduled in memory order so the mesh streams through L2 exactly once.
+//     brick (or half of one).  Readout: the brick's gathers hit the same few mesh rows, which therefore
+//     stay in that SM's L1; bricks are scheduled in memory order so the mesh streams through L2 exactly
+//     once; the streamed per-particle operands arrive through a cp.async ring (rkd_pipelined_kernel,
+//     brick_gather_kernel) and the force components are interleaved per cell (one 16-byte gather).
 //   * Paint: global fp32 reductions are bounded by the L2 atomic units (measured ~0.6 T RED/s, 8 per
 //     particle), so the brick accumulates into a shared-memory window placed at its mean
 //     displacement and flushes the window with one 16-byte vector reduction per 4 cells
