@@ -141,10 +141,12 @@ paint_direct_kernel(const float* __restrict__ pos, const float* __restrict__ mas
 // ---- paint: brick window in shared memory ----------------------------------------------------------
 // Window of the brick (resolution factor 1): brick extent + kHalo cells either side + 1 (CIC reaches
 // the next cell); z is padded so the origin can be rounded down to a multiple of 4 cells.
-constexpr int kHalo = 4;
+// Halo swept at C4 over the whole 40-step schedule (paint ms/step): 4 -> 1.034, 3 -> 1.001, 2 -> 0.986,
+// 1 -> 1.016 (more particles take the slow path); late steps (a > 0.9): 1.137 / - / 1.117 / 1.190.
+constexpr int kHalo = 2;
 constexpr int WX = BX + 2 * kHalo + 1, WY = BY + 2 * kHalo + 1;
 constexpr int WZ = (BZ + 2 * kHalo + 1 + 3 + 3) & ~3;
-constexpr int kWinCells = WX * WY * WZ;       // 17 x 25 x 44 = 18700 cells, 74.8 KB
+constexpr int kWinCells = WX * WY * WZ;       // 13 x 21 x 40 = 10920 cells, 43.7 KB
 
 template <bool FIXED, bool HAS_MASS>
 __global__ void __launch_bounds__(kBrickThreads, 2)
