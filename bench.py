@@ -63,7 +63,7 @@ def algorithmic_bytes(n_p, ng):
 
 def ncu_traffic(config):
     """{kernel: dram__bytes_read.sum + dram__bytes_write.sum per launch} from profiles/ncu_traffic.csv
-    (written from the `ncu --set full` capture named in its last column; see profiles/r01_C_C4.md)."""
+    (written from the `ncu --set full` capture named in its last column, e.g. profiles/r01_D_C4.md)."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     out = {}
     if os.path.exists(path):
