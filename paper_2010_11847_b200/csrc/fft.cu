@@ -29,8 +29,12 @@ PlanInfo plan_info(int n) {
 }
 
 // stage s >= 1: table[(t-1) NS + k] = exp(-2 pi i t k / (NS R_s)), t = 1..R_s-1, k < NS
-void build_stage_table(int n, std::vector<float2>& out) {
-  const PlanInfo pi = plan_info(n);
+PlanInfo plan_info_x(int n) {      // plan of the fused x round trip (fft_x_force_kernel)
+  if (n == 512) return Plan<512, 1>::info();
+  return plan_info(n);
+}
+
+void build_stage_table(const PlanInfo& pi, std::vector<float2>& out) {
   int ns = pi.r[0];
   for (int s = 1; s < pi.nst; ++s) {
     const int r = pi.r[s];
@@ -161,8 +165,8 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     e = set_smem(kern, xf_smem_bytes<N>());
     if (e != cudaSuccess) return e;
     const int ncols = N * nzh;
-    kern<<<(ncols + TX - 1) / TX, TX * Plan<N>::P, xf_smem_bytes<N>(), s>>>(
-        dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_n, kt.lap, kt.grad, scale);
+    kern<<<(ncols + TX - 1) / TX, TX * Plan<N, xf_variant<N>()>::P, xf_smem_bytes<N>(), s>>>(
+        dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_x, kt.lap, kt.grad, scale);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
@@ -202,9 +206,11 @@ bool fft_size_supported(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 
 
 cudaError_t fft_tables_create(int n, FftTables* out) {
   std::vector<float2> host;
-  build_stage_table(n, host);
+  build_stage_table(plan_info(n), host);
   const size_t off_m = host.size();
-  build_stage_table(n / 2, host);
+  build_stage_table(plan_info(n / 2), host);
+  const size_t off_x = host.size();
+  build_stage_table(plan_info_x(n), host);
   const size_t off_f = host.size();
   for (int k = 0; k < n / 2; ++k) {
     const double ang = -2.0 * kPi * k / n;
@@ -219,6 +225,7 @@ cudaError_t fft_tables_create(int n, FftTables* out) {
   out->dev = dev;
   out->stage_n = dev;
   out->stage_m = dev + off_m;
+  out->stage_x = dev + off_x;
   out->full = dev + off_f;
   return cudaSuccess;
 }

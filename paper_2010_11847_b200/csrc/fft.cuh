@@ -99,9 +99,12 @@ struct PlanInfo {
   int n, e, nst, r[3];
 };
 
-template <int N> struct Plan;
-#define FPM_PLAN(N_, E_, NST_, R0_, R1_, R2_)                                        \
-  template <> struct Plan<N_> {                                                      \
+// V = 0: the default plan of a size; V = 1: an alternative with fewer points per thread (more resident
+// warps, one more shared-memory exchange) for kernels that run several transforms per tile.
+template <int N, int V = 0> struct Plan;
+#define FPM_PLAN(N_, E_, NST_, R0_, R1_, R2_) FPM_PLAN_V(N_, 0, E_, NST_, R0_, R1_, R2_)
+#define FPM_PLAN_V(N_, V_, E_, NST_, R0_, R1_, R2_)                                  \
+  template <> struct Plan<N_, V_> {                                                      \
     static constexpr int E = E_, NST = NST_, R0 = R0_, R1 = R1_, R2 = R2_;           \
     static constexpr int P = N_ / E_;                                                \
     __host__ __device__ static constexpr int radix(int s) { return s == 0 ? R0_ : (s == 1 ? R1_ : R2_); } \
@@ -121,7 +124,9 @@ FPM_PLAN(128, 16, 2, 16, 8, 1)
 FPM_PLAN(256, 16, 2, 16, 16, 1)
 FPM_PLAN(512, 32, 2, 32, 16, 1)
 FPM_PLAN(1024, 32, 2, 32, 32, 1)
+FPM_PLAN_V(512, 1, 8, 3, 8, 8, 8)
 #undef FPM_PLAN
+#undef FPM_PLAN_V
 
 // shared-memory accessors -----------------------------------------------------------------
 // column tile: element i of column c at i*T + c (lanes run over c: conflict-free)
@@ -145,10 +150,9 @@ __host__ __device__ constexpr int row_pitch(int m) { return m + (m >> 4) + 1; }
 // Stage with radix R, NS lines already combined: butterfly j reads x[j + t N/R], multiplies by
 // exp(-2 pi i t k/(NS R)), k = j mod NS, and writes y[(j-k) R + k + t NS].
 // ------------------------------------------------------------------------------------------
-template <int N, int S, class SM>
-__device__ __forceinline__ void fft_stage(float2 (&v)[Plan<N>::E], const int p, const SM& sm,
+template <class PL, int S, class SM>
+__device__ __forceinline__ void fft_stage(float2 (&v)[PL::E], const int p, const SM& sm,
                                           const float2* __restrict__ tw) {
-  using PL = Plan<N>;
   constexpr int E = PL::E, P = PL::P, R = PL::radix(S), NS = PL::ns(S), M = E / R;
   constexpr bool last = (S == PL::NST - 1);
 #pragma unroll
@@ -178,7 +182,7 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[Plan<N>::E], const int p, 
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = sm.ld(p + P * e);
     if constexpr (S + 1 < PL::NST - 1) __syncthreads();
-    fft_stage<N, S + 1, SM>(v, p, sm, tw);
+    fft_stage<PL, S + 1, SM>(v, p, sm, tw);
   }
 }
 
@@ -186,7 +190,13 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[Plan<N>::E], const int p, 
 template <int N, class SM>
 __device__ __forceinline__ void fft_line(float2 (&v)[Plan<N>::E], const int p, const SM& sm,
                                          const float2* __restrict__ tw) {
-  fft_stage<N, 0, SM>(v, p, sm, tw);
+  fft_stage<Plan<N>, 0, SM>(v, p, sm, tw);
+}
+// the same with an explicit plan (tw must be that plan's stage table)
+template <class PL, class SM>
+__device__ __forceinline__ void fft_line_plan(float2 (&v)[PL::E], const int p, const SM& sm,
+                                              const float2* __restrict__ tw) {
+  fft_stage<PL, 0, SM>(v, p, sm, tw);
 }
 
 }  // namespace fpm

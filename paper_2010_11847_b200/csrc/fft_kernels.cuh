@@ -67,18 +67,21 @@ fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
 // columns = flattened (y, kz), lines = x with stride line_stride; no normalisation here.
 // Tile of TX columns; shared memory = [exchange N*TX | parked spectrum N*TX] float2.
 template <int N> __host__ __device__ constexpr int xf_tile() { return N >= 512 ? 8 : col_tile<N>(); }
+// plan variant of the x round trip: three transforms per tile make it compute-latency bound, so at
+// N = 512 it runs the 8-points-per-thread plan (32 instead of 12 resident warps per SM)
+template <int N> __host__ __device__ constexpr int xf_variant() { return N == 512 ? 1 : 0; }
 template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
   return sizeof(float2) * 2 * (size_t)N * xf_tile<N>();
 }
 
 template <int N>
-__global__ void __launch_bounds__(xf_tile<N>() * Plan<N>::P)
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P)
 fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
                    float2* __restrict__ out_bx, int ncols, int nzh, int64_t line_stride,
                    const float2* __restrict__ tw, const float* __restrict__ lap,
                    const float* __restrict__ grad, float scale) {
   extern __shared__ float2 smem[];
-  using PL = Plan<N>;
+  using PL = Plan<N, xf_variant<N>()>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
   const int64_t col = (int64_t)blockIdx.x * T + c;
@@ -88,7 +91,7 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
   for (int e = 0; e < E; ++e)
     v[e] = ok ? in[col + (int64_t)(p + P * e) * line_stride] : make_float2(0.f, 0.f);
   ColSmem<T> sm{smem, c};
-  fft_line<N>(v, p, sm, tw);
+  fft_line_plan<PL>(v, p, sm, tw);
   const int y = ok ? (int)(col / nzh) : 0, kz = ok ? (int)(col % nzh) : 0;
   const float lyz = __ldg(lap + y) + __ldg(lap + kz);
   float2* park = smem + N * T + threadIdx.x;          // element e of this thread at park[e * T * P]
@@ -102,7 +105,7 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
     park[e * (T * P)] = v[e];
   }
   if constexpr (PL::NST > 1) __syncthreads();
-  fft_line<N>(v, p, sm, tw);
+  fft_line_plan<PL>(v, p, sm, tw);
   if (ok) {
 #pragma unroll
     for (int e = 0; e < E; ++e) out_a[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
@@ -114,7 +117,7 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
     v[e] = make_float2(a.x * g, a.y * g);
   }
   if constexpr (PL::NST > 1) __syncthreads();
-  fft_line<N>(v, p, sm, tw);
+  fft_line_plan<PL>(v, p, sm, tw);
   if (ok) {
 #pragma unroll
     for (int e = 0; e < E; ++e) out_bx[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);

@@ -44,9 +44,10 @@ struct ProfScope {
 // ---- FFT (fft.cu) ---------------------------------------------------------------------------
 struct FftTables {
   int n = 0;
-  float2* dev = nullptr;       // one allocation: [stage table N][stage table N/2][W_N^k, k < N/2]
+  float2* dev = nullptr;       // one allocation: [stage table N][stage table N/2][stage table x plan][W_N^k, k < N/2]
   float2* stage_n = nullptr;
   float2* stage_m = nullptr;
+  float2* stage_x = nullptr;   // stage table of the plan fft_x_force_kernel uses (may equal stage_n's)
   float2* full = nullptr;
 };
 cudaError_t fft_tables_create(int n, FftTables* out);
