@@ -172,12 +172,16 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   {
     ProfScope sc(prof, K_FFT_Y_INV3);
+    using YPL = Plan<N, yi_variant<N>()>;
+    constexpr int TY = yi_tile<N>();
+    const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
     auto kern = fft_y_inv3_kernel<N>;
-    e = set_smem(kern, smem);
+    e = set_smem(kern, ysmem);
     if (e != cudaSuccess) return e;
-    dim3 grid(3 * ((nzh + T - 1) / T), N);
+    dim3 grid(3 * ((nzh + TY - 1) / TY), N);
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    kern<<<grid, threads, smem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * nzh, nzh, nzh, t.stage_n, kt.grad);
+    kern<<<grid, TY * YPL::P, ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * nzh, nzh, nzh,
+                                         yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }

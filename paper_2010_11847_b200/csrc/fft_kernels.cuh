@@ -127,15 +127,18 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
 // The three inverse y passes of the fused force path in one launch.  Block b: tile b / 3 of x slab
 // blockIdx.y, variant b % 3:  0: Bx -> Fx (in place),  1: g(w_y) A -> Fy,  2: A -> Fz (g(w_z) is applied
 // by the z pass).  in0/out0 may alias; A is read by variants 1 and 2 and written by neither.
+template <int N> __host__ __device__ constexpr int yi_tile() { return N == 512 ? 8 : col_tile<N>(); }
+template <int N> __host__ __device__ constexpr int yi_variant() { return N == 512 ? 1 : 0; }
+
 template <int N>
-__global__ void __launch_bounds__(col_tile<N>() * Plan<N>::P, cols_min_blocks<N>())
+__global__ void __launch_bounds__(yi_tile<N>() * Plan<N, yi_variant<N>()>::P)
 fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
                   float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
                   int ncols, int64_t line_stride, const float2* __restrict__ tw,
                   const float* __restrict__ grad) {
   extern __shared__ float2 smem[];
-  using PL = Plan<N>;
-  constexpr int T = col_tile<N>(), E = PL::E, P = PL::P;
+  using PL = Plan<N, yi_variant<N>()>;
+  constexpr int T = yi_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
   const int variant = blockIdx.x % 3;
   const int64_t col = (int64_t)(blockIdx.x / 3) * T + c;
@@ -153,7 +156,7 @@ fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* 
     v[e] = cswap(x);
   }
   ColSmem<T> sm{smem, c};
-  fft_line<N>(v, p, sm, tw);
+  fft_line_plan<PL>(v, p, sm, tw);
   if (ok) {
 #pragma unroll
     for (int e = 0; e < E; ++e) out[off + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
