@@ -63,7 +63,7 @@ def algorithmic_bytes(n_p, ng):
 
 def ncu_traffic(config):
     """{kernel: dram__bytes_read.sum + dram__bytes_write.sum per launch} from profiles/ncu_traffic.csv
-    (written from the `ncu --set full` capture named in its last column, e.g. profiles/r01_D_C4.md)."""
+    (written from the `ncu --set full` capture named in its last column, e.g. profiles/r01_E_C4.md)."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     out = {}
     if os.path.exists(path):
@@ -103,7 +103,13 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.monotonic(), [c.strip() for c in line.split(",")]))
+
+    def mark_begin(self):
+        self.t_begin = time.monotonic()
+
+    def mark_end(self):
+        self.t_end = time.monotonic()
 
     def stop(self):
         if not self.proc:
@@ -116,7 +122,13 @@ class ClockSampler:
             self.proc.kill()
         sm, smax, reasons, power = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        # samples taken while the timed region ran (nvidia-smi is started before the warm-up so that it is
+        # already streaming); if the region was shorter than the sampling period, the nearest samples
+        t0, t1 = getattr(self, "t_begin", None), getattr(self, "t_end", None)
+        rows = [r for t, r in self.rows if t0 is None or (t0 <= t <= t1 + 0.05)]
+        if len(rows) < 2 and t0 is not None:
+            rows = [r for _, r in sorted(self.rows, key=lambda tr: abs(tr[0] - 0.5 * (t0 + t1)))[:3]]
+        for r in rows:
             if len(r) < 7:
                 continue
             try:
@@ -303,6 +315,9 @@ def main():
     def fac(i):  # beyond the schedule keep stepping with the last full step's factors
         return factors[i] if i < len(factors) - 1 else factors[len(factors) - 2]
 
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
     step_no = 0
     for _ in range(args.warmup):
         ctx.pm_step(pos, mom, *fac(step_no))
@@ -311,9 +326,7 @@ def main():
     rep.barrier()
     torch.cuda.synchronize()
 
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
+    sampler.mark_begin()
     ctx.profile_reset()
     ctx.profile_enable(True)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -326,6 +339,7 @@ def main():
     torch.cuda.synchronize()
     rep.barrier()
     torch.cuda.synchronize()
+    sampler.mark_end()
     ms_total = ev0.elapsed_time(ev1)
     launches = ctx.launch_count()
     prof = ctx.profile_read()
