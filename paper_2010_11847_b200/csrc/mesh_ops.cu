@@ -219,9 +219,11 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   const int oz = (qz0 + mz - kHalo) & ~3;
   // Fixed point with a power-of-two scale 2^floor(log2(2^18 / mmax)) (exact for weights that are dyadic
   // fractions).  No cell can overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2)
-  // <= 2^30 + 2^11 < 2^31.
-  const float scale = FIXED ? (mmax > 0.f ? __int_as_float(__float_as_int((float)(1 << 18) / mmax) & 0x7F800000) : 0.f)
-                            : 1.f;
+  // <= 2^30 + 2^11 < 2^31.  With one positive mass for all particles (the density paint of a run) every
+  // deposit is >= 0, the window is read back as unsigned and the scale is 2^19: sums < 2^31 + 2^11 < 2^32.
+  const bool nonneg = !HAS_MASS && mass_const > 0.f;
+  const float top = nonneg ? (float)(1 << 19) : (float)(1 << 18);
+  const float scale = FIXED ? (mmax > 0.f ? __int_as_float(__float_as_int(top / mmax) & 0x7F800000) : 0.f) : 1.f;
 
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
@@ -280,7 +282,11 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
     if (FIXED) {
       const int4 q = reinterpret_cast<const int4*>(win_i)[gidx];
       any = (q.x | q.y | q.z | q.w) != 0;
-      v = make_float4(q.x * inv_scale, q.y * inv_scale, q.z * inv_scale, q.w * inv_scale);
+      if (nonneg)
+        v = make_float4(__uint2float_rn((unsigned)q.x) * inv_scale, __uint2float_rn((unsigned)q.y) * inv_scale,
+                        __uint2float_rn((unsigned)q.z) * inv_scale, __uint2float_rn((unsigned)q.w) * inv_scale);
+      else
+        v = make_float4(q.x * inv_scale, q.y * inv_scale, q.z * inv_scale, q.w * inv_scale);
     } else {
       v = reinterpret_cast<const float4*>(win_f)[gidx];
       any = !(v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f);
