@@ -144,15 +144,26 @@ int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, con
   { ProfScope sc2(pr, K_READOUT_GRAD);
     if (brick) FPM_CUDA(ctx, force_vjp_direct_brick(w.rho, pos, v, (float)coef, n, ng, gx, ord, s));
     else FPM_CUDA(ctx, readout3_grad_accum(w.F[0], w.F[1], w.F[2], pos, v, (float)coef, n, ng, gx, s)); }
-  // ... and the cotangent of the meshes: Fbar_d = paint(pos, mass = v_d)
-  for (int d = 0; d < 3; ++d) {
-    { ProfScope sc2(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.rho, true, ord, s)); }
-    FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.fk[d], s, pr));
+  // ... and the cotangent of the meshes: Fbar_d = paint(pos, mass = v_d);
+  // rho_bar = sum_d M_d^T Fbar_d = -sum_d M_d Fbar_d  (M_d odd and imaginary in k-space)
+  if (ctx->cfg.kernel_mode != FPM_KERNEL_NAIVE) {
+    // Eq. 5's i g(w) is the symbol of the 4-point difference D, so sum_d i g_d Fbar_d,k is the transform of
+    // the real-space stencil divergence: three paints, one stencil pass, ONE potential solve.
+    for (int d = 0; d < 3; ++d) {
+      ProfScope sc2(pr, K_PAINT);
+      FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.F[d], true, ord, s));
+    }
+    { ProfScope sc2(pr, K_GREEN); FPM_CUDA(ctx, stencil_divergence(w.F[0], w.F[1], w.F[2], ng, w.rho, s)); }
+    FPM_CUDA(ctx, fft_poisson(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.F[0], (float)(-coef * sc), s, pr));
+  } else {
+    for (int d = 0; d < 3; ++d) {
+      { ProfScope sc2(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.rho, true, ord, s)); }
+      FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.fk[d], s, pr));
+    }
+    { ProfScope sc2(pr, K_GREEN);
+      FPM_CUDA(ctx, apply_force_kernel_transpose(ctx->kt_g, w.fk[0], w.fk[1], w.fk[2], (float)(coef * sc), w.dk, s)); }
+    FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.dk, w.F[0], s, pr));
   }
-  // rho_bar = sum_d M_d^T Fbar_d = -sum_d M_d Fbar_d
-  { ProfScope sc2(pr, K_GREEN);
-    FPM_CUDA(ctx, apply_force_kernel_transpose(ctx->kt_g, w.fk[0], w.fk[1], w.fk[2], (float)(coef * sc), w.dk, s)); }
-  FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.dk, w.F[0], s, pr));
   // rho = paint(pos, m): cotangent of pos = m sum_c rho_bar[c] dW/dx
   ProfScope sc2(pr, K_READOUT_GRAD);
   if (brick_walk_ok(n, ord, pos, gx, nullptr))

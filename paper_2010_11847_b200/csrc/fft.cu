@@ -204,6 +204,50 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   return launch_z_c2r<N>(t, wc, F[2], kt.grad, s, prof);
 }
 
+// real mesh -> real mesh:  out = c2r[ (scale / K^2) r2c[src] ]  (K^2 of the context's kernel mode, 0 at k = 0),
+// with the multiplier fused into the x round trip; work: one half-complex scratch buffer.
+template <int N>
+cudaError_t poisson_impl(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
+                         float scale, cudaStream_t s, Profiler* prof) {
+  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
+  const int64_t nrows = (int64_t)N * N;
+  cudaError_t e;
+  {
+    ProfScope sc(prof, K_FFT_Z_R2C);
+    constexpr int threads = G * Plan<M>::P;
+    const size_t smem = sizeof(float2) * G * row_pitch(M);
+    auto kern = fft_z_r2c_kernel<N>;
+    e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(src, work, nrows, t.stage_m, t.full);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  {
+    ProfScope sc(prof, K_FFT_Y);
+    e = launch_cols<N, false>(work, work, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    if (e != cudaSuccess) return e;
+  }
+  {
+    ProfScope sc(prof, K_FFT_X_FORCE);
+    constexpr int TX = xf_tile<N>();
+    auto kern = fft_x_force_kernel<N, true>;
+    e = set_smem(kern, xf_smem_bytes<N>());
+    if (e != cudaSuccess) return e;
+    const int ncols = N * nzh;
+    kern<<<(ncols + TX - 1) / TX, TX * Plan<N, xf_variant<N>()>::P, xf_smem_bytes<N>(), s>>>(
+        work, work, nullptr, ncols, nzh, (int64_t)N * nzh, t.stage_x, kt.lap, kt.grad, scale);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  {
+    ProfScope sc(prof, K_FFT_Y);
+    e = launch_cols<N, true>(work, work, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    if (e != cudaSuccess) return e;
+  }
+  return launch_z_c2r<N>(t, work, out, nullptr, s, prof);
+}
+
 }  // namespace
 
 bool fft_size_supported(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
@@ -258,6 +302,12 @@ cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStr
 }
 cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s, Profiler* prof) {
   FPM_FFT_DISPATCH(c2r_impl, t, cplx, real, s, prof)
+}
+
+cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
+                        float scale, cudaStream_t s, Profiler* prof) {
+  if (kt.n != t.n) return cudaErrorInvalidValue;
+  FPM_FFT_DISPATCH(poisson_impl, t, kt, src, work, out, scale, s, prof)
 }
 
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,

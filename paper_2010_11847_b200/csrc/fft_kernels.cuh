@@ -74,9 +74,11 @@ template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
   return sizeof(float2) * 2 * (size_t)N * xf_tile<N>();
 }
 
-template <int N>
+// POISSON: only  out_a = inverse_x[ (scale / K^2) forward_x[in] ]  (real multiplier, no gradient variant;
+// out_a may alias in) -- the x round trip of the backward pass's single potential solve.
+template <int N, bool POISSON = false>
 __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P)
-fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
+fft_x_force_kernel(const float2* in, float2* out_a,
                    float2* __restrict__ out_bx, int ncols, int nzh, int64_t line_stride,
                    const float2* __restrict__ tw, const float* __restrict__ lap,
                    const float* __restrict__ grad, float scale) {
@@ -100,9 +102,13 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
     const int i = p + P * e;
     const float k2 = __ldg(lap + i) + lyz;
     const float f = (col == 0 && i == 0) ? 0.f : scale / k2;
-    // i f v = (-im, re) f ; kept (im, re)-swapped for the inverse transform
-    v[e] = make_float2(v[e].x * f, -v[e].y * f);
-    park[e * (T * P)] = v[e];
+    if constexpr (POISSON) {
+      v[e] = make_float2(v[e].y * f, v[e].x * f);        // f v, (im, re)-swapped
+    } else {
+      // i f v = (-im, re) f ; kept (im, re)-swapped for the inverse transform
+      v[e] = make_float2(v[e].x * f, -v[e].y * f);
+      park[e * (T * P)] = v[e];
+    }
   }
   if constexpr (PL::NST > 1) __syncthreads();
   fft_line_plan<PL>(v, p, sm, tw);
@@ -110,6 +116,7 @@ fft_x_force_kernel(const float2* __restrict__ in, float2* __restrict__ out_a,
 #pragma unroll
     for (int e = 0; e < E; ++e) out_a[col + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
   }
+  if constexpr (POISSON) return;
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const float g = __ldg(grad + p + P * e);

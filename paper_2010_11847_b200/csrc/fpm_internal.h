@@ -81,6 +81,10 @@ cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const fl
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
                             cudaStream_t s, Profiler* prof = nullptr);
 
+// out = c2r[(scale / K^2) r2c[src]] with the multiplier fused into the x round trip (backward pass)
+cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
+                        float scale, cudaStream_t s, Profiler* prof = nullptr);
+
 // ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
 // How the caller's particle arrays are ordered: np > 0 says "n == np^3 particles in lattice
 // (Lagrangian) order", which lets the kernels walk them brick by brick; results never depend on it.
@@ -131,6 +135,8 @@ cudaError_t lpt_spectral(const KernelTables& kt, const float2* in, float2* out, 
 // backward pass: out_k = - sum_d (i scale g_d / K^2) f_d,k  (= sum_d M_d^T)
 cudaError_t apply_force_kernel_transpose(const KernelTables& kt, const float2* f0, const float2* f1,
                                          const float2* f2, float scale, float2* out, cudaStream_t s);
+// g = sum_d D_d f_d, D the periodic 4-point central difference whose symbol is i g(w) of Eq. 5
+cudaError_t stencil_divergence(const float* f0, const float* f1, const float* f2, int n, float* g, cudaStream_t s);
 cudaError_t axpy(float* y, const float* x, float a, int64_t n, cudaStream_t s);            // y += a x
 cudaError_t lincomb2(float* out, const float* a, float ca, const float* b, float cb, int64_t n,
                      cudaStream_t s);                                                        // ca a + cb b

@@ -132,6 +132,26 @@ lpt_source_kernel(float* __restrict__ s, const float* __restrict__ a, const floa
   }
 }
 
+// g[c] = sum_d (D_d f_d)[c],  (D f)[i] = (-f[i+2] + 8 f[i+1] - 8 f[i-1] + f[i-2]) / 12 along axis d, periodic.
+// D has the symbol i g(w) of PAPER.md Eq. 5, so r2c(g) = sum_d i g_d r2c(f_d): the backward pass forms
+// this sum in real space and runs ONE potential solve instead of three forward transforms (R12).
+__global__ void __launch_bounds__(256)
+stencil_divergence_kernel(const float* __restrict__ f0, const float* __restrict__ f1,
+                          const float* __restrict__ f2, int n, float* __restrict__ g) {
+  const int mask = n - 1;
+  const int z = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y, x = blockIdx.z;
+  if (z >= n) return;
+  const int64_t row = ((int64_t)x * n + y) * n;
+  auto at = [&](const float* f, int xx, int yy, int zz) {
+    return __ldg(f + ((int64_t)(xx & mask) * n + (yy & mask)) * n + (zz & mask));
+  };
+  const float dx = -at(f0, x + 2, y, z) + 8.f * at(f0, x + 1, y, z) - 8.f * at(f0, x - 1, y, z) + at(f0, x - 2, y, z);
+  const float dy = -at(f1, x, y + 2, z) + 8.f * at(f1, x, y + 1, z) - 8.f * at(f1, x, y - 1, z) + at(f1, x, y - 2, z);
+  const float dz = -at(f2, x, y, z + 2) + 8.f * at(f2, x, y, z + 1) - 8.f * at(f2, x, y, z - 1) + at(f2, x, y, z - 2);
+  g[row + z] = (dx + dy + dz) * (1.f / 12.f);
+}
+
 // y += a x
 __global__ void __launch_bounds__(256)
 axpy_kernel(float* __restrict__ y, const float* __restrict__ x, float a, int64_t n) {
@@ -222,6 +242,13 @@ cudaError_t apply_force_kernel_transpose(const KernelTables& kt, const float2* f
                                          const float2* f2, float scale, float2* out, cudaStream_t s) {
   force_kernel_transpose_rows<<<(unsigned)(kt.n * kt.n), kThreads, 0, s>>>(f0, f1, f2, kt.n, kt.lap,
                                                                           kt.grad, scale, out);
+  return cudaGetLastError();
+}
+
+cudaError_t stencil_divergence(const float* f0, const float* f1, const float* f2, int n, float* g, cudaStream_t s) {
+  const int bt = n < 256 ? n : 256;
+  dim3 grid((n + bt - 1) / bt, n, n);
+  stencil_divergence_kernel<<<grid, bt, 0, s>>>(f0, f1, f2, n, g);
   return cudaGetLastError();
 }
 
