@@ -135,21 +135,36 @@ lpt_source_kernel(float* __restrict__ s, const float* __restrict__ a, const floa
 // g[c] = sum_d (D_d f_d)[c],  (D f)[i] = (-f[i+2] + 8 f[i+1] - 8 f[i-1] + f[i-2]) / 12 along axis d, periodic.
 // D has the symbol i g(w) of PAPER.md Eq. 5, so r2c(g) = sum_d i g_d r2c(f_d): the backward pass forms
 // this sum in real space and runs ONE potential solve instead of three forward transforms (R12).
+// A block owns a 64 (z) x 4 (y) tile and walks kStencilXC planes along x, so the x-difference needs one
+// new load per cell and plane (five-deep register ring) and the y / z neighbours come from L1.
+constexpr int kStencilXC = 32;
 __global__ void __launch_bounds__(256)
 stencil_divergence_kernel(const float* __restrict__ f0, const float* __restrict__ f1,
                           const float* __restrict__ f2, int n, float* __restrict__ g) {
   const int mask = n - 1;
-  const int z = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y, x = blockIdx.z;
-  if (z >= n) return;
-  const int64_t row = ((int64_t)x * n + y) * n;
-  auto at = [&](const float* f, int xx, int yy, int zz) {
-    return __ldg(f + ((int64_t)(xx & mask) * n + (yy & mask)) * n + (zz & mask));
-  };
-  const float dx = -at(f0, x + 2, y, z) + 8.f * at(f0, x + 1, y, z) - 8.f * at(f0, x - 1, y, z) + at(f0, x - 2, y, z);
-  const float dy = -at(f1, x, y + 2, z) + 8.f * at(f1, x, y + 1, z) - 8.f * at(f1, x, y - 1, z) + at(f1, x, y - 2, z);
-  const float dz = -at(f2, x, y, z + 2) + 8.f * at(f2, x, y, z + 1) - 8.f * at(f2, x, y, z - 1) + at(f2, x, y, z - 2);
-  g[row + z] = (dx + dy + dz) * (1.f / 12.f);
+  const int z = blockIdx.x * 64 + (threadIdx.x & 63);
+  const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  if (z >= n || y >= n) return;
+  const int x0 = blockIdx.z * kStencilXC;
+  const int xc = n - x0 < kStencilXC ? n - x0 : kStencilXC;
+  const int64_t nn = (int64_t)n * n;
+  const int64_t yz = (int64_t)y * n + z;
+  const int zm2 = (z - 2) & mask, zm1 = (z - 1) & mask, zp1 = (z + 1) & mask, zp2 = (z + 2) & mask;
+  const int64_t ym2 = (int64_t)((y - 2) & mask) * n + z, ym1 = (int64_t)((y - 1) & mask) * n + z,
+                yp1 = (int64_t)((y + 1) & mask) * n + z, yp2 = (int64_t)((y + 2) & mask) * n + z;
+  float am2 = __ldg(f0 + (int64_t)((x0 - 2) & mask) * nn + yz), am1 = __ldg(f0 + (int64_t)((x0 - 1) & mask) * nn + yz);
+  float a0 = __ldg(f0 + (int64_t)x0 * nn + yz), ap1 = __ldg(f0 + (int64_t)((x0 + 1) & mask) * nn + yz);
+  for (int i = 0; i < xc; ++i) {
+    const int x = x0 + i;
+    const int64_t pl = (int64_t)x * nn;
+    const float ap2 = __ldg(f0 + (int64_t)((x + 2) & mask) * nn + yz);
+    const float dx = -ap2 + 8.f * ap1 - 8.f * am1 + am2;
+    const float dy = -__ldg(f1 + pl + yp2) + 8.f * __ldg(f1 + pl + yp1) - 8.f * __ldg(f1 + pl + ym1) + __ldg(f1 + pl + ym2);
+    const int64_t row = pl + (int64_t)y * n;
+    const float dz = -__ldg(f2 + row + zp2) + 8.f * __ldg(f2 + row + zp1) - 8.f * __ldg(f2 + row + zm1) + __ldg(f2 + row + zm2);
+    g[pl + yz] = (dx + dy + dz) * (1.f / 12.f);
+    am2 = am1; am1 = a0; a0 = ap1; ap1 = ap2;
+  }
 }
 
 // y += a x
@@ -246,9 +261,8 @@ cudaError_t apply_force_kernel_transpose(const KernelTables& kt, const float2* f
 }
 
 cudaError_t stencil_divergence(const float* f0, const float* f1, const float* f2, int n, float* g, cudaStream_t s) {
-  const int bt = n < 256 ? n : 256;
-  dim3 grid((n + bt - 1) / bt, n, n);
-  stencil_divergence_kernel<<<grid, bt, 0, s>>>(f0, f1, f2, n, g);
+  dim3 grid((n + 63) / 64, (n + 3) / 4, (n + kStencilXC - 1) / kStencilXC);
+  stencil_divergence_kernel<<<grid, 256, 0, s>>>(f0, f1, f2, n, g);
   return cudaGetLastError();
 }
 
