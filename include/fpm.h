@@ -21,6 +21,11 @@
  *     k-space meshes are [ng][ng][ng/2+1] interleaved complex64 (the cuFFT r2c layout), integer
  *     frequency n_d in (-ng/2, ng/2], omega_d = 2 pi n_d / ng.
  *   - Sizes: ng and np are powers of two, 8 <= np <= ng <= 1024, ng % np == 0.
+ *   - Performance paths (results never depend on them): when n == np^3 particles are passed in lattice
+ *     (Lagrangian) order -- what fpm_lpt_init produces and every later call preserves -- with np a
+ *     multiple of 32 and 16-byte aligned arrays, paint, readout and the fused step walk the particles brick
+ *     by brick (shared-memory paint window, cp.async-pipelined gathers); any other particle set takes the
+ *     generic one-thread-per-particle kernels.
  */
 #ifndef FPM_H
 #define FPM_H
