@@ -28,6 +28,20 @@ def test_force_vjp_matches_oracle(fpm, oracle, ng, nps, n, force_path):
     assert rel_l2(got, ref) < TOL
 
 
+@pytest.mark.parametrize("mode", [1, 2])
+def test_force_vjp_other_kernel_modes(fpm, oracle, mode):
+    """NAIVE (i k, -1/k^2) takes the three-transform adjoint path, MIXED the stencil-divergence path."""
+    ng = nps = 32
+    n = nps ** 3
+    pos = fi.random_particles(n, ng, 23, clustered=True)
+    v = np.random.default_rng(24).standard_normal((3, n)).astype(np.float32)
+    for force_path in (0, 1):
+        ctx = fpm.FPM(ng, nps, kernel_mode=mode, force_path=force_path)
+        got = host(ctx.force_vjp(dev(pos), dev(v), coef=1.3))
+        ref = 1.3 * oracle.force_vjp(pos.astype(np.float64), ng, v.astype(np.float64), mode=mode, scale=1.5 * OM)
+        assert rel_l2(got, ref) < TOL
+
+
 def test_force_vjp_accumulates_into_grad_pos(fpm):
     ng, n = 16, 500
     pos = dev(fi.random_particles(n, ng, 5))
