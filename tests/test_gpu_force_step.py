@@ -178,3 +178,19 @@ def test_full_run_C2_matches_oracle(fpm, oracle):
     k, pk_ref, nm = oracle.power(oracle.paint(rpos, cfg.ng), cfg.box)
     _, pk_got, _ = oracle.power(oracle.paint(pos.astype(np.float64), cfg.ng), cfg.box)
     assert np.max(np.abs(pk_got / pk_ref - 1)) < 1e-4
+
+
+def test_full_run_naive_kernel_and_quinn_factors(fpm, oracle):
+    """C1 through the fused path with the other option of each switch: -1/k^2, ik kernels (R3d) and the
+    plain Quinn et al. kick/drift integrals (R4)."""
+    cfg = fi.CONFIGS["C1"]
+    delta = fi.linear_field(cfg.np_side, cfg.box, cfg.seed)
+    ctx = fpm.FPM(cfg.ng, cfg.np_side, box=cfg.box, kernel_mode=fpm.KERNEL_NAIVE, factor_mode=fpm.FACTORS_QUINN,
+                  force_path=1)
+    pos, mom = ctx.lpt_init(dev(delta), cfg.a0, cfg.lpt_order)
+    p0, m0 = host(pos).astype(np.float64), host(mom).astype(np.float64)
+    ctx.nbody(pos, mom, cfg.stages())
+    rpos, rmom = oracle.nbody(p0, m0, cfg.ng, cfg.np_side, OM, cfg.stages(), mode=oracle.KERNEL_NAIVE,
+                              factor_mode=oracle.FACTORS_QUINN)
+    assert periodic_dist(host(pos), rpos, cfg.ng).max() < 1e-3
+    assert rel_l2(host(mom), rmom) < 1e-4
