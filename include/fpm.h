@@ -66,7 +66,7 @@ enum {
 
 /* How fpm_paint scatters (results agree within fp32 summation order). */
 enum {
-  FPM_PAINT_AUTO = 0,        /* brick window when the particles are a full np^3 lattice set, ng == np */
+  FPM_PAINT_AUTO = 0,        /* brick window when the particles are a full np^3 lattice set, ng == np or 2 np */
   FPM_PAINT_DIRECT = 1,      /* one thread per particle, 8 global fp32 reductions */
   FPM_PAINT_BRICK_FLOAT = 2, /* shared-memory window per lattice brick, fp32 accumulation */
   FPM_PAINT_BRICK_FIXED = 3  /* shared-memory window per lattice brick, 32-bit fixed-point accumulation */

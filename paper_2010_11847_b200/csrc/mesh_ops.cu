@@ -148,29 +148,38 @@ constexpr int WX = BX + 2 * kHalo + 1, WY = BY + 2 * kHalo + 1;
 constexpr int WZ = (BZ + 2 * kHalo + 1 + 3 + 3) & ~3;
 constexpr int kWinCells = WX * WY * WZ;       // 13 x 21 x 40 = 10920 cells, 43.7 KB
 
-template <bool FIXED, bool HAS_MASS>
+// RES = ng / np (1 or 2): the lattice spacing in cells.  The CTA's sub-brick of (8 x 16 x 32) / RES lattice
+// sites always spans 8 x 16 x 32 cells, so the window is the same; with RES = 2 a thread owns one particle.
+template <bool FIXED, bool HAS_MASS, int RES = 1>
 __global__ void __launch_bounds__(kBrickThreads, 2)
 paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
                    int64_t n, BrickMap bm, int ng, float* __restrict__ mesh) {
+  constexpr int SX = BX / RES, SY = BY / RES, SZ = BZ / RES;          // lattice sites of the sub-brick
+  constexpr int kPerThread = SX * SY * SZ / kBrickThreads;
+  static_assert(kPerThread >= 1 && SX % kPerThread == 0, "sub-brick shape");
   extern __shared__ __align__(16) float win_f[];
   int* win_i = reinterpret_cast<int*>(win_f);
   __shared__ float red[4][kBrickThreads / 32];
   const int mask = ng - 1;
   const float fng = (float)ng, inv_ng = 1.f / fng;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int qx0, qy0, qz0;
-  bm.origin(blockIdx.x, qx0, qy0, qz0);
+  // sub-brick origin (lattice sites) and this thread's first site: slot s = tid + 512 k has offsets
+  // lz = s % SZ, ly = (s / SZ) % SY, lx = s / (SZ SY)  (RES = 1: lz = lane, ly = warp, lx = k)
+  const int nbz = bm.np / SZ, nby = bm.np / SY;
+  const int qz0 = (int)(blockIdx.x % nbz) * SZ, qy0 = (int)((blockIdx.x / nbz) % nby) * SY,
+            qx0 = (int)(blockIdx.x / nbz / nby) * SX;
+  const int lz = tid % SZ, ly = (tid / SZ) % SY, lx0 = tid / (SZ * SY);
+  constexpr int kDx = kBrickThreads / (SZ * SY);     // lattice planes advanced per k
 
   for (int i = tid; i < kWinCells / 4; i += kBrickThreads)
     reinterpret_cast<float4*>(win_f)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
-  // this thread's particles (slot s = tid + 512 k: lattice offsets lz = lane, ly = warp, lx = k)
   float x[kPerThread], y[kPerThread], z[kPerThread], m[HAS_MASS ? kPerThread : 1];
-  const int64_t p0 = bm.index(qx0, qy0, qz0, tid);
   const int64_t plane = (int64_t)bm.np * bm.np;
+  const int64_t p0 = ((int64_t)(qx0 + lx0) * bm.np + (qy0 + ly)) * bm.np + (qz0 + lz);
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
-    const int64_t p = p0 + k * plane;
+    const int64_t p = p0 + (int64_t)(k * kDx) * plane;
     x[k] = ld_stream(pos + p);
     y[k] = ld_stream(pos + n + p);
     z[k] = ld_stream(pos + 2 * n + p);
@@ -178,14 +187,14 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   }
   // mean displacement from the lattice sites (wrapped to [-ng/2, ng/2)) places the window
   float sx = 0.f, sy = 0.f, sz = 0.f, mmax = HAS_MASS ? 0.f : fabsf(mass_const);
-  const float qy = (float)(qy0 + warp), qz = (float)(qz0 + lane);
+  const float qy = (float)((qy0 + ly) * RES), qz = (float)((qz0 + lz) * RES);    // lattice site in cells
   // (a sample of kMeanPlanes of the brick's x planes is enough: the window position only decides how
   //  many particles take the slow path, never the result)
-  constexpr int kMeanPlanes = 2, kMeanStep = kPerThread / kMeanPlanes;
+  constexpr int kMeanPlanes = kPerThread >= 2 ? 2 : 1, kMeanStep = kPerThread / kMeanPlanes;
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
     if (k % kMeanStep == 0) {
-      float dx = x[k] - (float)(qx0 + k), dy = y[k] - qy, dz = z[k] - qz;
+      float dx = x[k] - (float)((qx0 + lx0 + k * kDx) * RES), dy = y[k] - qy, dz = z[k] - qz;
       int unused;
       dx -= fng * fast_rint(dx * inv_ng, unused);
       dy -= fng * fast_rint(dy * inv_ng, unused);
@@ -214,15 +223,20 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   fast_floor(sx * inv_cnt, mx);
   fast_floor(sy * inv_cnt, my);
   fast_floor(sz * inv_cnt, mz);
-  const int ox = qx0 + mx - kHalo;
-  const int oy = qy0 + my - kHalo;
-  const int oz = (qz0 + mz - kHalo) & ~3;
+  const int ox = qx0 * RES + mx - kHalo;
+  const int oy = qy0 * RES + my - kHalo;
+  const int oz = (qz0 * RES + mz - kHalo) & ~3;
   // Fixed point with a power-of-two scale 2^floor(log2(2^18 / mmax)) (exact for weights that are dyadic
   // fractions).  No cell can overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2)
   // <= 2^30 + 2^11 < 2^31.  With one positive mass for all particles (the density paint of a run) every
   // deposit is >= 0, the window is read back as unsigned and the scale is 2^19: sums < 2^31 + 2^11 < 2^32.
+  // (in general 2^30 resp. 2^31 over the particles per CTA, capped at 2^21: the magic-number rounding
+  // needs |deposit| < 2^22; a RES = 2 sub-brick holds 512 particles and reaches the cap)
   const bool nonneg = !HAS_MASS && mass_const > 0.f;
-  const float top = nonneg ? (float)(1 << 19) : (float)(1 << 18);
+  constexpr int kPerCta = SX * SY * SZ;
+  constexpr float kTopSigned = (float)((1 << 30) / kPerCta < (1 << 21) ? (1 << 30) / kPerCta : (1 << 21));
+  constexpr float kTopUnsigned = 2.f * kTopSigned < (float)(1 << 21) ? 2.f * kTopSigned : (float)(1 << 21);
+  const float top = nonneg ? kTopUnsigned : kTopSigned;
   const float scale = FIXED ? (mmax > 0.f ? __int_as_float(__float_as_int(top / mmax) & 0x7F800000) : 0.f) : 1.f;
 
 #pragma unroll
@@ -702,7 +716,8 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
   }
   if (n == 0) return cudaSuccess;
   int mode = ord.paint_mode;
-  const bool can_brick = brick_ok(n, ord.np) && ng == ord.np && ng % 4 == 0 &&
+  const int res = ord.np > 0 ? ng / ord.np : 0;
+  const bool can_brick = brick_ok(n, ord.np) && (res == 1 || res == 2) && ng == res * ord.np && ng % 4 == 0 &&
                          (reinterpret_cast<uintptr_t>(mesh) & 15) == 0;
   if (mode == FPM_PAINT_AUTO) mode = can_brick ? FPM_PAINT_BRICK_FIXED : FPM_PAINT_DIRECT;
   if (mode != FPM_PAINT_DIRECT && !can_brick) mode = FPM_PAINT_DIRECT;
@@ -711,7 +726,7 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
     return cudaGetLastError();
   }
   const size_t smem = sizeof(float) * (size_t)kWinCells;
-  const unsigned grid = (unsigned)(n / kBrick);
+  const unsigned grid = (unsigned)(n / (kBrick / (res * res * res)));
   const BrickMap bm = brick_map(ord.np);
   auto go = [&](auto kern) -> cudaError_t {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -719,6 +734,11 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
     kern<<<grid, kBrickThreads, smem, s>>>(pos, mass, mass_const, n, bm, ng, mesh);
     return cudaGetLastError();
   };
+  if (res == 2) {
+    if (mode == FPM_PAINT_BRICK_FIXED)
+      return mass ? go(paint_brick_kernel<true, true, 2>) : go(paint_brick_kernel<true, false, 2>);
+    return mass ? go(paint_brick_kernel<false, true, 2>) : go(paint_brick_kernel<false, false, 2>);
+  }
   if (mode == FPM_PAINT_BRICK_FIXED)
     return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
   return mass ? go(paint_brick_kernel<false, true>) : go(paint_brick_kernel<false, false>);

@@ -91,3 +91,26 @@ def test_adjoints_match_oracle_and_dot_product_identity(fpm, oracle):
     lhs = float((ctx.paint(dev(pos), dev(m)).double() * dev(gbar).double()).sum())
     rhs = float((dev(m).double() * ctx.readout(dev(gbar), dev(pos)).double()).sum())
     assert lhs == pytest.approx(rhs, rel=1e-5)
+
+
+@pytest.mark.parametrize("mode", ["fixed", "float"])
+def test_brick_paint_with_resolution_factor_two(fpm, oracle, mode):
+    """A full lattice particle set on a mesh twice as fine (C3's regime: 1/8 particle per cell) takes
+    the sub-brick window path; displaced lattice with a few multi-cell outliers, against the oracle."""
+    import paper_2010_11847_b200 as m
+    nps, ng = 32, 64
+    n = nps ** 3
+    rng = np.random.default_rng(7)
+    q = np.stack(np.meshgrid(*[np.arange(nps) * 2.0] * 3, indexing="ij")).reshape(3, n)
+    pos = q + rng.normal(0.0, 0.8, size=(3, n))
+    pos[:, ::97] += rng.normal(0.0, 6.0, size=(3, len(range(0, n, 97))))     # outliers leave the window
+    pos = np.mod(pos, ng).astype(np.float32)
+    ctx = m.FPM(ng, nps, paint_mode=m.PAINT_BRICK_FIXED if mode == "fixed" else m.PAINT_BRICK_FLOAT)
+    got = host(ctx.paint(dev(pos)))
+    ref = oracle.paint(pos.astype(np.float64), ng, mass_const=8.0)
+    assert rel_l2(got, ref) < TOL
+    assert abs(got.astype(np.float64).sum() - 8.0 * n) < 1e-5 * 8.0 * n
+    mass = rng.standard_normal(n).astype(np.float32)                         # signed per-particle masses
+    got = host(ctx.paint(dev(pos), mass=dev(mass)))
+    ref = oracle.paint(pos.astype(np.float64), ng, mass=mass.astype(np.float64))
+    assert rel_l2(got, ref) < TOL
