@@ -65,20 +65,33 @@ def ncu_traffic(config):
     """{kernel: dram__bytes_read.sum + dram__bytes_write.sum per launch} from profiles/ncu_traffic.csv
     (written from the `ncu --set full` capture named in its last column, e.g. profiles/r01_E_C4.md)."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
-    out = {}
+    out, src = {}, {}
     if os.path.exists(path):
         with open(path) as f:
             next(f)
             for line in f:
-                cfg, kernel, nbytes, _ = line.strip().split(",")
+                cfg, kernel, nbytes, capture = line.strip().split(",")
                 if cfg == config:
                     out[kernel] = int(nbytes)
-    return out
+                    src[kernel] = capture
+    return out, src
 
 
 def step_bytes_unfused(n_p, ng):
     """SURVEY.md 8(d) unfused model: 96 n_p + 112 n_g bytes per PM step."""
     return 96 * n_p + 112 * ng ** 3
+
+
+def step_bytes_fused_path(n_p, ng):
+    """Compulsory bytes of the fused path as built: 60 n_p + 88 n_g = the sum of the seven
+    kernels' algorithmic bytes + the 8 n_g of the interleaved force cell's pad (written and read, not credited
+    per kernel)."""
+    return 60 * n_p + 88 * ng ** 3
+
+
+def step_bytes_fused_bound(n_p, ng):
+    """SURVEY.md 8(d) "fused lower bound": 60 n_p + 104 n_g."""
+    return 60 * n_p + 104 * ng ** 3
 
 
 class ClockSampler:
@@ -146,47 +159,59 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None}
 
 
-def oracle_sample(cfg, n_side, n_steps):
-    """Times the float64 oracle on n_steps PM steps of an n_side^3 slice of the workload."""
+def oracle_sample(cfg, n_side, n_steps, ng_side=None):
+    """Times the float64 oracle on n_steps PM steps (paint, r2c, Eq. 3-5, 3 c2r, 3 readouts, kick, drift --
+    each an oracle call, nothing tuned) of an n_side^3-particle slice of the workload with the workload's
+    particle spacing and mesh resolution (n_side = np_side: the workload itself), from 1LPT ICs."""
     import oracle
+    ng_side = n_side * cfg.resolution_factor if ng_side is None else ng_side
     box = cfg.box * n_side / cfg.np_side          # same particle spacing as the workload
     delta = fi.linear_field(n_side, box, cfg.seed).astype(np.float64)
     om = fi.COSMO["omega_m"]
-    pos, mom = oracle.lpt_init(delta, n_side, om, cfg.a0, 1)
+    pos, mom = oracle.lpt_init(delta, ng_side, om, cfg.a0, 1)
+    del delta
     stages = cfg.stages()
+    mass = float(cfg.resolution_factor ** 3)
     times = []
     for j in range(n_steps):
         ai, af = stages[j], stages[j + 1]
         ah = (ai * af) ** 0.5
         t0 = time.perf_counter()
-        f = oracle.force(pos, n_side, scale=1.5 * om, mass=1.0)
+        f = oracle.force(pos, ng_side, scale=1.5 * om, mass=mass)
         mom = oracle.kick(mom, f, oracle.kick_factor(om, ai, ai, ah))
-        pos = oracle.drift(pos, mom, oracle.drift_factor(om, ai, ah, af), n_side)
+        pos = oracle.drift(pos, mom, oracle.drift_factor(om, ai, ah, af), ng_side)
         times.append(time.perf_counter() - t0)
     return times, oracle.num_threads()
 
 
 def run_reference(args):
-    """--impl reference: the oracle as it stands on the host cores, same metric and unit."""
+    """--impl reference: the oracle as it stands on the host cores, same metric, unit and workload.  One
+    oracle PM step at 512^3 takes most of a minute, so the requested --steps / --warmup are CAPPED to what ends
+    within a few minutes (default: 2 timed steps, no warm-up -- a CPU program has nothing to warm); the line
+    says how many were really run, and `ms_per_step` is what was measured, not an extrapolation."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     cfg = fi.CONFIGS[args.config]
-    n_side = min(cfg.np_side, 256 if args.ref_side is None else args.ref_side)
-    total = args.steps + args.warmup
-    times, cores = oracle_sample(cfg, n_side, total)
-    timed = times[args.warmup:]
-    upd_per_s = n_side ** 3 * len(timed) / sum(timed)
-    value = upd_per_s / cfg.n_particles
-    sample = (f"{len(timed)} PM steps (+{args.warmup} warm-up) of a {n_side}^3-particle / {n_side}^3-mesh slice "
-              f"of {cfg.name} (same particle spacing), float64 oracle; steps/s scaled by particle count "
-              f"{n_side}^3/{cfg.np_side}^3")
+    n_side = cfg.np_side if args.ref_side is None else min(cfg.np_side, args.ref_side)
+    cap = args.ref_max_steps
+    steps, warmup = max(1, min(args.steps, cap)), min(args.warmup, max(0, cap - min(args.steps, cap)))
+    times, cores = oracle_sample(cfg, n_side, steps + warmup)
+    timed = times[warmup:]
+    frac = (n_side / cfg.np_side) ** 3
+    value = len(timed) / sum(timed) * frac        # steps/s of the workload (frac = 1: measured, not scaled)
+    sample = (f"{len(timed)} PM steps (+{warmup} warm-up; requested --steps {args.steps} --warmup {args.warmup}, capped "
+              f"to keep the run within minutes) of "
+              + (f"the full workload {cfg.name}" if frac == 1.0 else
+                 f"a {n_side}^3-particle slice of {cfg.name} (same particle spacing; steps/s scaled by {frac:g})")
+              + ", float64 oracle, 1LPT ICs")
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": "steps/s",
-        "particle_updates_per_sec": upd_per_s, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
+        "particle_updates_per_sec": value * cfg.n_particles, "n_gpus": args.gpus, "steps": len(timed),
+        "warmup": warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "sample": sample},
+        "config": {"workload": workload_name(cfg), "sample": sample, "requested_steps": args.steps,
+                   "requested_warmup": args.warmup, "ms_per_step_measured": [1e3 * t for t in timed]},
         "cpu_baseline": {"value": value, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -276,32 +301,44 @@ def side_measurements(args, ctx, cfg, pos, mom, factors, device):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=37)   # + 3 warm-up = C4's 40-step schedule
+    ap.add_argument("--steps", type=int, default=None, help="timed PM steps (default: the rest of the schedule)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=sorted(fi.CONFIGS))
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-side", action="store_true", help="skip the cuFFT floor and backward-step timings")
-    ap.add_argument("--ref-side", type=int, default=None)
+    ap.add_argument("--no-side", action="store_true", help="skip the cuFFT floor, whole-run, backward and N1/N2 timings")
+    ap.add_argument("--ref-side", type=int, default=None, help="--impl reference: run a slice of this many particles per side")
+    ap.add_argument("--ref-max-steps", type=int, default=2, help="--impl reference: cap on steps + warm-up really run")
     ap.add_argument("--force-path", default="fused", choices=["fused", "unfused"])
     args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = fi.CONFIGS[args.config]
+    n_sched = cfg.n_steps + 1          # PM steps (force evaluations) of the whole schedule
     if args.impl == "reference":
+        args.steps = 20 if args.steps is None else args.steps
         run_reference(args)
         return
+    args.warmup = max(args.warmup, 3)
+    if args.steps is None:
+        args.steps = n_sched - args.warmup
+    if args.warmup + args.steps > n_sched or args.steps < 1:
+        ap.error(f"--warmup {args.warmup} + --steps {args.steps} exceeds the {n_sched} PM steps of {cfg.name}'s schedule "
+                 f"(the timed steps walk the real schedule; nothing is repeated)")
+
+    from paper_2010_11847_b200 import replicas as rep
+    if rep.needs_spawn(args.gpus):
+        # `python bench.py --gpus N` outside torchrun: start the N replica ranks (one process per GPU)
+        sys.exit(subprocess.call(rep.launch_command(args.gpus, os.path.abspath(__file__), sys.argv[1:])))
 
     import torch
 
     import paper_2010_11847_b200 as fpm   # raises if libfpm.so is missing: no fallback
-    from paper_2010_11847_b200 import replicas as rep
 
     rank, local_rank, world = rep.env_world()
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
     rep.init("nccl", device)
 
-    cfg = fi.CONFIGS[args.config]
     n_p, ng = cfg.n_particles, cfg.ng
     ctx = fpm.FPM(ng, cfg.np_side, omega_m=fi.COSMO["omega_m"], box=cfg.box, device=device,
                   force_path=fpm.FORCE_FUSED if args.force_path == "fused" else fpm.FORCE_UNFUSED)
@@ -309,18 +346,15 @@ def main():
     # ---- inputs: seeded Gaussian field -> 2LPT particles, all resident in HBM -----------------
     delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, rep.replica_seed(cfg.seed, rank))).to(device)
     pos, mom = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
-    del delta
-    factors = ctx.step_factors(cfg.stages())
-
-    def fac(i):  # beyond the schedule keep stepping with the last full step's factors
-        return factors[i] if i < len(factors) - 1 else factors[len(factors) - 2]
+    stages = cfg.stages()
+    factors = ctx.step_factors(stages)          # fpm_step_factors: the schedule arithmetic is behind the C-ABI
 
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     step_no = 0
     for _ in range(args.warmup):
-        ctx.pm_step(pos, mom, *fac(step_no))
+        ctx.pm_step(pos, mom, *factors[step_no])
         step_no += 1
     torch.cuda.synchronize()
     rep.barrier()
@@ -333,7 +367,7 @@ def main():
     ev0.record()
     first_timed = step_no
     for _ in range(args.steps):
-        ctx.pm_step(pos, mom, *fac(step_no))
+        ctx.pm_step(pos, mom, *factors[step_no])
         step_no += 1
     ev1.record()
     torch.cuda.synchronize()
@@ -350,20 +384,24 @@ def main():
     value = rep.whole_job_rate(args.steps, ms_total, world)     # whole-job steps/s (replicas)
 
     # ---- end to end through the C-ABI with HOST buffers -----------------------------------------
+    # (continues the schedule where it has steps left, else repeats its last full step: the state is the
+    #  clustered end-of-run one either way, and this leg is dominated by the PCIe copies)
     e2e = None
     if args.e2e_steps > 0:
+        def e2e_fac(i):
+            return factors[min(i, n_sched - 2)]
         h_pos = torch.empty((3, n_p), dtype=torch.float32, pin_memory=True)
         h_mom = torch.empty((3, n_p), dtype=torch.float32, pin_memory=True)
         h_pos.copy_(pos)
         h_mom.copy_(mom)
         torch.cuda.synchronize()
-        ctx.pm_step_host(h_pos, h_mom, pos, mom, *fac(step_no))   # warm-up
+        ctx.pm_step_host(h_pos, h_mom, pos, mom, *e2e_fac(step_no))   # warm-up
         step_no += 1
         rep.barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(args.e2e_steps):
-            ctx.pm_step_host(h_pos, h_mom, pos, mom, *fac(step_no))
+            ctx.pm_step_host(h_pos, h_mom, pos, mom, *e2e_fac(step_no))
             step_no += 1
         e1.record()
         torch.cuda.synchronize()
@@ -375,7 +413,26 @@ def main():
                "call": "fpm_pm_step_host (pinned host pos+mom -> device, step, -> host)"}
         del h_pos, h_mom
 
-    extras = side_measurements(args, ctx, cfg, pos, mom, fac(step_no), device) if (rank == 0 and world == 1) else {}
+    # ---- the whole run as ONE C call: fpm_nbody over every force evaluation of the schedule ------------
+    whole_run = None
+    if not args.no_side:
+        pos2, mom2 = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
+        torch.cuda.synchronize()
+        rep.barrier()
+        w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0.record()
+        ctx.nbody(pos2, mom2, stages)
+        w1.record()
+        torch.cuda.synchronize()
+        ms_run = rep.max_over_ranks(w0.elapsed_time(w1), device)
+        whole_run = {"call": "fpm_nbody (2LPT state -> a = 1), CUDA events around the one call",
+                     "force_evaluations": n_sched, "ms": ms_run, "ms_per_step": ms_run / n_sched,
+                     "steps_per_s": rep.whole_job_rate(n_sched, ms_run, world)}
+        del pos2, mom2
+    del delta
+
+    extras = side_measurements(args, ctx, cfg, pos, mom, factors[min(step_no, n_sched - 2)], device) \
+        if (rank == 0 and world == 1) else {}
 
     if rank != 0:
         rep.finalize()
@@ -396,8 +453,7 @@ def main():
             k["frac"] = k["gbs"] / peak
         kernels[name] = k
     dominant = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
-    traffic = None
-    traffic_table = ncu_traffic(args.config)     # per-launch DRAM bytes from the committed ncu capture
+    traffic_table, traffic_src = ncu_traffic(args.config)     # per-launch DRAM bytes from the committed ncu capture
     traffic = traffic_table.get(dominant)
     for name, k in kernels.items():
         if name in traffic_table:
@@ -405,11 +461,21 @@ def main():
     dk = kernels[dominant]
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk.get("gbs"), "peak": peak,
                 "unit": "GB/s", "frac": dk.get("frac"), "traffic": traffic, "peak_source": peak_src,
+                "traffic_source": (f"profiles/ncu_traffic.csv, capture {traffic_src.get(dominant)} (an earlier ncu --set "
+                                   f"full run of this command, not this run)") if traffic is not None else None,
                 "share_of_step": dk["ms_per_step"] / ms_per_step}
-    step_gbs = step_bytes_unfused(n_p, ng) / ms_per_step / 1e6
-    step_roofline = {"algorithmic_bytes_per_step": step_bytes_unfused(n_p, ng), "achieved": step_gbs,
-                     "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
-                     "model": "96 n_p + 112 n_g (SURVEY.md 8(d), unfused)"}
+    own, bound, unf = step_bytes_fused_path(n_p, ng), step_bytes_fused_bound(n_p, ng), step_bytes_unfused(n_p, ng)
+    fused = args.force_path == "fused"
+    step_roofline = {"unit": "GB/s", "peak": peak,
+                     "algorithmic_bytes_per_step": own if fused else unf,
+                     "achieved": (own if fused else unf) / ms_per_step / 1e6,
+                     "frac": (own if fused else unf) / ms_per_step / 1e6 / peak,
+                     "model": ("60 n_p + 88 n_g: the compulsory bytes of the fused path as built (DESIGN.md 6)" if fused
+                               else "96 n_p + 112 n_g (SURVEY.md 8(d), unfused)"),
+                     "frac_vs_survey_fused_bound": bound / ms_per_step / 1e6 / peak,
+                     "survey_fused_bound_bytes": bound,
+                     "vs_unfused_model": {"bytes": unf, "frac": unf / ms_per_step / 1e6 / peak,
+                                          "note": "bytes the fused path never moves; context only"}}
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
@@ -417,9 +483,10 @@ def main():
         times, cores = oracle_sample(cfg, side, 3)
         upd = side ** 3 * 2 / sum(times[1:])
         cpu_baseline = {"value": upd / n_p, "unit": "steps/s", "cores": cores, "kind": "oracle",
-                        "particle_updates_per_sec": upd,
-                        "sample": f"2 PM steps (+1 warm-up) of a {side}^3-particle / {side}^3-mesh slice of "
-                                  f"{cfg.name}, float64 oracle, steps/s scaled by {side}^3/{cfg.np_side}^3"}
+                        "particle_updates_per_sec": upd, "ms_per_sample_step": [1e3 * t for t in times[1:]],
+                        "sample": f"2 PM steps (+1 warm-up) of a {side}^3-particle / {side * cfg.resolution_factor}^3-mesh "
+                                  f"slice of {cfg.name} (same particle spacing), float64 oracle; steps/s scaled by "
+                                  f"{side}^3/{cfg.np_side}^3 (`bench.py --impl reference` times the full-size step)"}
 
     out = {
         "metric": METRIC, "value": value, "unit": "steps/s",
@@ -428,12 +495,13 @@ def main():
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": workload_name(cfg), "timed_schedule_steps": [first_timed, first_timed + args.steps - 1],
+                   "schedule_pm_steps": n_sched,
                    "l2_policy": "inputs larger than L2 (3.2 GB particle state, 0.5 GB meshes vs 126 MB L2)",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "kernel_mode": "paper Eq. 4+5", "force_path": args.force_path},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
-        "cpu_baseline": cpu_baseline,
+        "whole_run": whole_run, "cpu_baseline": cpu_baseline,
     }
     out.update(extras)
     print(json.dumps(out), flush=True)

@@ -21,11 +21,14 @@
  *     k-space meshes are [ng][ng][ng/2+1] interleaved complex64 (the cuFFT r2c layout), integer
  *     frequency n_d in (-ng/2, ng/2], omega_d = 2 pi n_d / ng.
  *   - Sizes: ng and np are powers of two, 8 <= np <= ng <= 1024, ng % np == 0.
- *   - Performance paths (results never depend on them): when n == np^3 particles are passed in lattice
- *     (Lagrangian) order -- what fpm_lpt_init produces and every later call preserves -- with np a
- *     multiple of 32 and 16-byte aligned arrays, paint, readout and the fused step walk the particles brick
- *     by brick (shared-memory paint window, cp.async-pipelined gathers); any other particle set takes the
- *     generic one-thread-per-particle kernels.
+ *   - Performance paths: when n == np^3 particles are passed in lattice (Lagrangian) order -- what
+ *     fpm_lpt_init produces and every later call preserves -- with np a multiple of 32 and 16-byte aligned
+ *     arrays, paint, readout and the fused step walk the particles brick by brick (shared-memory paint
+ *     window, cp.async-pipelined gathers); any other particle set takes the generic one-thread-per-particle
+ *     kernels.  Gathers give the same values either way; for paint see FPM_PAINT_* below (the brick window
+ *     is fixed point, within the stated quantum of the direct fp32 reductions).
+ *   - Device: a context belongs to the CUDA device that was current in fpm_create; every later call runs
+ *     there whatever device is current in the calling thread (which is restored on return).
  */
 #ifndef FPM_H
 #define FPM_H
@@ -64,9 +67,16 @@ enum {
   FPM_FORCE_FUSED = 1    /* Green's function fused into the FFT passes, readout+kick+drift fused */
 };
 
-/* How fpm_paint scatters (results agree within fp32 summation order). */
+/* How fpm_paint scatters.  DIRECT and BRICK_FLOAT agree within fp32 summation order.  BRICK_FIXED rounds every
+ * deposit m_p W to a multiple of a per-brick (4096 lattice neighbours, 512 when ng = 2 np) power-of-two
+ * quantum q: q <= 2^-19 m for the density paint of a run (mass == NULL), and
+ * q <= max(2^-18 mean|m|, 2^-21 max|m|) over the brick with per-particle masses; a cell is off by at most
+ * q/2 per deposit it receives (measured 1.5e-6 relative L2 on the density).  A brick holding a non-finite
+ * mass, or whose max|m| exceeds 64 mean|m|, is deposited with plain fp32 reductions instead (so NaN/Inf
+ * propagate and an outlier does not coarsen its neighbours).  Particles a brick's window cannot hold always
+ * take plain fp32 reductions: the result is defined for any input. */
 enum {
-  FPM_PAINT_AUTO = 0,        /* brick window when the particles are a full np^3 lattice set, ng == np or 2 np */
+  FPM_PAINT_AUTO = 0,        /* BRICK_FIXED when the particles are a full np^3 lattice set and ng == np or 2 np, else DIRECT */
   FPM_PAINT_DIRECT = 1,      /* one thread per particle, 8 global fp32 reductions */
   FPM_PAINT_BRICK_FLOAT = 2, /* shared-memory window per lattice brick, fp32 accumulation */
   FPM_PAINT_BRICK_FIXED = 3  /* shared-memory window per lattice brick, 32-bit fixed-point accumulation */
@@ -112,6 +122,14 @@ int fpm_growth(const fpm_ctx* ctx, double a, double* out);
  * force (epoch a_c) to move p from a_i to a_f.  HOST doubles. */
 int fpm_drift_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out);
 int fpm_kick_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out);
+/* The (kick_fac, drift_fac) pairs of the n_steps + 1 PM steps fpm_nbody performs for the schedule
+ * a_stages[0 .. n_steps]: the half step sits at sqrt(a_j a_j+1), and the
+ * two half kicks that use the same force evaluation are merged, so step j is
+ *   mom += f(pos) * kick_fac[j];  pos = wrap(pos + mom * drift_fac[j]),   drift_fac[n_steps] = 0.
+ * a_stages, kick_fac, drift_fac: HOST double arrays of n_steps + 1 entries.  fpm_nbody, fpm_nbody_vjp and
+ * fpm_pm_step callers all use exactly these numbers. */
+int fpm_step_factors(const fpm_ctx* ctx, const double* a_stages, int n_steps, double* kick_fac,
+                     double* drift_fac);
 
 /* ---- the operators of one PM step --------------------------------------------------------- */
 
@@ -124,7 +142,13 @@ int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, floa
  * unnormalised.  real [ng^3] is read only; cplx [ng*ng*(ng/2+1)] complex64 (float2). */
 int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx);
 /* Inverse: real(x) = ng^-3 sum_k cplx(k) exp(+2 pi i n.x/ng), with the
- * Hermitian half implied.  cplx is CLOBBERED (used as scratch for the in-place passes). */
+ * Hermitian half implied.  cplx is CLOBBERED (used as scratch for the in-place passes).
+ * Input contract: cplx is the half-complex spectrum of a REAL field, i.e. on the planes kz = 0 and
+ * kz = ng/2 it satisfies cplx(-kx, -ky, kz) = conj(cplx(kx, ky, kz)) (true of every spectrum this library
+ * produces: fpm_fft_r2c output times a transfer function with the parity of Eq. 3-5).  On other inputs the
+ * result is the real part of the inverse transform of the spectrum completed by
+ * cplx(-kx, -ky, -kz) := conj(cplx(kx, ky, kz)) for 0 < kz < ng/2 and taken as stored on those two planes:
+ * the component of the two planes that breaks the symmetry contributes its real part only. */
 int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real);
 
 /* Transfer function (Eq. 3-5): fk_d = scale * i g(omega_d) delta_k / K^2,
@@ -208,9 +232,12 @@ int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, dou
 /* Reverse of fpm_nbody.  traj: DEVICE [(n_steps+1)][3][n] as stored by fpm_nbody for the same HOST
  * a_stages.  grad_pos / grad_mom: DEVICE [3][n]; on entry dL/d(final pos, final mom), on return
  * dL/d(initial pos, initial mom) (updated in place).  The forward force meshes of every step are
- * recomputed from traj. */
+ * recomputed from traj.  flags: 0, or FPM_VJP_GRAD_MOM_ZERO when the caller guarantees that grad_mom is all
+ * zeros on entry (a loss on the final positions only): the force VJP of the last force evaluation, which
+ * then adds exactly zero, is skipped (one of n_steps + 1 backward force evaluations). */
+enum { FPM_VJP_GRAD_MOM_ZERO = 1 };
 int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n_steps,
-                  float* grad_pos, float* grad_mom);
+                  float* grad_pos, float* grad_mom, int flags);
 
 /* Reverse of fpm_lpt_init.  grad_pos / grad_mom: DEVICE [3][np^3] (read only); grad_delta: DEVICE
  * [np^3] = dL/d(delta_lin) (overwritten).  delta_lin, a0, order as in the forward call. */

@@ -18,6 +18,7 @@ KERNEL_PAPER, KERNEL_NAIVE, KERNEL_MIXED = 0, 1, 2
 FACTORS_FASTPM, FACTORS_QUINN = 0, 1
 FORCE_UNFUSED, FORCE_FUSED = 0, 1
 PAINT_AUTO, PAINT_DIRECT, PAINT_BRICK_FLOAT, PAINT_BRICK_FIXED = 0, 1, 2, 3
+VJP_GRAD_MOM_ZERO = 1
 OK, EINVAL, ENOMEM, ECUDA, ENOTIMPL = 0, -1, -2, -3, -4
 
 
@@ -51,6 +52,7 @@ def _load():
         "fpm_growth": (i32, [vp, dbl, ctypes.POINTER(dbl)]),
         "fpm_drift_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
         "fpm_kick_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
+        "fpm_step_factors": (i32, [vp, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]),
         "fpm_paint": (i32, [vp, vp, vp, i64, vp]),
         "fpm_fft_r2c": (i32, [vp, vp, vp]),
         "fpm_fft_c2r": (i32, [vp, vp, vp]),
@@ -71,7 +73,7 @@ def _load():
                                    ctypes.POINTER(i64)]),
         "fpm_launch_count": (i64, [vp]),
         "fpm_force_vjp": (i32, [vp, vp, i64, vp, dbl, vp]),
-        "fpm_nbody_vjp": (i32, [vp, vp, ctypes.POINTER(dbl), i32, vp, vp]),
+        "fpm_nbody_vjp": (i32, [vp, vp, ctypes.POINTER(dbl), i32, vp, vp, i32]),
         "fpm_lpt_init_vjp": (i32, [vp, vp, dbl, i32, vp, vp, vp]),
         "fpm_recon_scratch_bytes": (ctypes.c_size_t, [ctypes.POINTER(_Config), i32]),
         "fpm_recon_loss_grad": (i32, [vp, vp, vp, dbl, vp, ctypes.POINTER(dbl), i32, i32, vp, ctypes.c_size_t, vp,
@@ -97,13 +99,24 @@ def library_path():
     return _LIB_PATH
 
 
-def _dev(t, dtype=torch.float32):
+def _dev(t, dtype=torch.float32, numel=None, what="tensor"):
+    """data_ptr of a contiguous CUDA tensor of the given dtype (and element count, when the C call assumes
+    one): a wrong size would be an out-of-bounds device access behind the C-ABI, so it is refused here."""
     if t is None:
         return None
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
         raise FpmError(f"expected a contiguous CUDA {dtype} tensor (no CPU fallback), got "
                        f"{type(t).__name__} {getattr(t, 'dtype', None)} {getattr(t, 'device', None)}")
+    if numel is not None and t.numel() != numel:
+        raise FpmError(f"{what}: expected {numel} elements, got {t.numel()} (shape {tuple(t.shape)})")
     return ctypes.c_void_p(t.data_ptr())
+
+
+def _particles(t, what="pos"):
+    """[3][n] particle array -> n."""
+    if not (isinstance(t, torch.Tensor) and t.dim() == 2 and t.shape[0] == 3):
+        raise FpmError(f"{what}: expected a [3][n] tensor, got shape {tuple(getattr(t, 'shape', ()))}")
+    return int(t.shape[1])
 
 
 class FPM:
@@ -174,37 +187,50 @@ class FPM:
         return out.value
 
     # ---- operators ------------------------------------------------------------------------
+    # Every wrapper checks the element counts the C call assumes (a wrong shape would be a silent
+    # out-of-bounds device access behind the C-ABI) and raises FpmError.
+    @property
+    def _n_g(self):
+        return self.ng ** 3
+
+    @property
+    def _n_k(self):
+        return self.ng * self.ng * self.nzh
+
     def paint(self, pos, mass=None, out=None):
-        n = pos.shape[1]
+        n = _particles(pos)
         mesh = out if out is not None else self._empty(self.ng, self.ng, self.ng)
-        self._check(_lib.fpm_paint(self._h, _dev(pos), _dev(mass), n, _dev(mesh)))
+        self._check(_lib.fpm_paint(self._h, _dev(pos), _dev(mass, numel=n, what="mass"), n,
+                                   _dev(mesh, numel=self._n_g, what="mesh")))
         return mesh
 
     def fft_r2c(self, real, out=None):
         cplx = out if out is not None else self._empty(self.ng, self.ng, self.nzh, dtype=torch.complex64)
-        self._check(_lib.fpm_fft_r2c(self._h, _dev(real), _dev(cplx, torch.complex64)))
+        self._check(_lib.fpm_fft_r2c(self._h, _dev(real, numel=self._n_g, what="real mesh"),
+                                     _dev(cplx, torch.complex64, self._n_k, "half-complex mesh")))
         return cplx
 
     def fft_c2r(self, cplx, out=None, clobber=False):
         work = cplx if clobber else cplx.clone()
         real = out if out is not None else self._empty(self.ng, self.ng, self.ng)
-        self._check(_lib.fpm_fft_c2r(self._h, _dev(work, torch.complex64), _dev(real)))
+        self._check(_lib.fpm_fft_c2r(self._h, _dev(work, torch.complex64, self._n_k, "half-complex mesh"),
+                                     _dev(real, numel=self._n_g, what="real mesh")))
         return real
 
     def apply_force_kernel(self, delta_k, scale=1.0):
         outs = [torch.empty_like(delta_k) for _ in range(3)]
-        self._check(_lib.fpm_apply_force_kernel(self._h, _dev(delta_k, torch.complex64), scale,
-                                                *[_dev(o, torch.complex64) for o in outs]))
+        self._check(_lib.fpm_apply_force_kernel(self._h, _dev(delta_k, torch.complex64, self._n_k, "delta_k"),
+                                                scale, *[_dev(o, torch.complex64) for o in outs]))
         return outs
 
     def readout(self, mesh, pos):
-        n = pos.shape[1]
+        n = _particles(pos)
         out = self._empty(n)
-        self._check(_lib.fpm_readout(self._h, _dev(mesh), _dev(pos), n, _dev(out)))
+        self._check(_lib.fpm_readout(self._h, _dev(mesh, numel=self._n_g, what="mesh"), _dev(pos), n, _dev(out)))
         return out
 
     def force(self, pos):
-        n = pos.shape[1]
+        n = _particles(pos)
         f = self._empty(3, n)
         self._check(_lib.fpm_force(self._h, _dev(pos), n, _dev(f)))
         return f
@@ -220,52 +246,58 @@ class FPM:
         return out
 
     def kick(self, mom, force, ai, ac, af):
-        self._check(_lib.fpm_kick(self._h, _dev(mom), _dev(force), mom.shape[1], ai, ac, af))
+        n = _particles(mom, "mom")
+        self._check(_lib.fpm_kick(self._h, _dev(mom), _dev(force, numel=3 * n, what="force"), n, ai, ac, af))
         return mom
 
     def drift(self, pos, mom, ai, ac, af):
-        self._check(_lib.fpm_drift(self._h, _dev(pos), _dev(mom), pos.shape[1], ai, ac, af))
+        n = _particles(pos)
+        self._check(_lib.fpm_drift(self._h, _dev(pos), _dev(mom, numel=3 * n, what="mom"), n, ai, ac, af))
         return pos
 
     def lpt_init(self, delta_lin, a0, order):
         pos, mom = self._empty(3, self.n_particles), self._empty(3, self.n_particles)
-        self._check(_lib.fpm_lpt_init(self._h, _dev(delta_lin), a0, order, _dev(pos), _dev(mom)))
+        self._check(_lib.fpm_lpt_init(self._h, _dev(delta_lin, numel=self.n_particles, what="delta_lin"), a0,
+                                      order, _dev(pos), _dev(mom)))
         return pos, mom
 
+    def _stages(self, stages):
+        if len(stages) < 1:
+            raise FpmError("stages: need at least a_0")
+        return (ctypes.c_double * len(stages))(*[float(a) for a in stages]), len(stages) - 1
+
     def nbody(self, pos, mom, stages, traj=None):
-        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
-        self._check(_lib.fpm_nbody(self._h, _dev(pos), _dev(mom), st, len(stages) - 1, _dev(traj)))
+        st, n_steps = self._stages(stages)
+        n3 = 3 * self.n_particles
+        self._check(_lib.fpm_nbody(self._h, _dev(pos, numel=n3, what="pos"), _dev(mom, numel=n3, what="mom"), st,
+                                   n_steps, _dev(traj, numel=(n_steps + 1) * n3, what="traj")))
         return pos, mom
 
     def pm_step(self, pos, mom, kick_fac, drift_fac):
         """One PM step: force at pos, mom += f * kick_fac, pos = wrap(pos + mom * drift_fac)."""
-        self._check(_lib.fpm_pm_step(self._h, _dev(pos), _dev(mom), pos.shape[1], kick_fac, drift_fac))
+        n = _particles(pos)
+        self._check(_lib.fpm_pm_step(self._h, _dev(pos), _dev(mom, numel=3 * n, what="mom"), n, kick_fac,
+                                     drift_fac))
         return pos, mom
 
     def pm_step_host(self, h_pos, h_mom, d_pos, d_mom, kick_fac, drift_fac):
         """The same step on HOST float32 tensors: H2D, step, D2H, synchronise."""
+        n = _particles(h_pos, "h_pos")
         for t in (h_pos, h_mom):
-            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
-                raise FpmError("pm_step_host expects contiguous CPU float32 tensors")
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or t.numel() != 3 * n:
+                raise FpmError("pm_step_host expects contiguous CPU float32 [3][n] tensors")
         self._check(_lib.fpm_pm_step_host(self._h, ctypes.c_void_p(h_pos.data_ptr()),
-                                          ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos), _dev(d_mom),
-                                          h_pos.shape[1], kick_fac, drift_fac))
+                                          ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos, numel=3 * n, what="d_pos"),
+                                          _dev(d_mom, numel=3 * n, what="d_mom"), n, kick_fac, drift_fac))
         return h_pos, h_mom
 
     def step_factors(self, stages):
-        """(kick_fac, drift_fac) of the n+1 PM steps fpm_nbody performs for stages a_0..a_n."""
-        out, pending = [], 0.0
-        n = len(stages) - 1
-        for j in range(n + 1):
-            kf, dr = pending, 0.0
-            if j < n:
-                ai, af = float(stages[j]), float(stages[j + 1])
-                ah = (ai * af) ** 0.5
-                kf += self.kick_factor(ai, ai, ah)
-                dr = self.drift_factor(ai, ah, af)
-                pending = self.kick_factor(ah, af, af)
-            out.append((kf, dr))
-        return out
+        """[(kick_fac, drift_fac)] of the n+1 PM steps fpm_nbody performs for stages a_0..a_n
+        (fpm_step_factors: the schedule arithmetic lives behind the C-ABI, not here)."""
+        st, n_steps = self._stages(stages)
+        kf, dr = (ctypes.c_double * (n_steps + 1))(), (ctypes.c_double * (n_steps + 1))()
+        self._check(_lib.fpm_step_factors(self._h, st, n_steps, kf, dr))
+        return list(zip(list(kf), list(dr)))
 
     # ---- measurement hooks ----------------------------------------------------------------
     def profile_enable(self, on=True):
@@ -291,65 +323,79 @@ class FPM:
 
     def nbody_host(self, h_pos, h_mom, d_pos, d_mom, stages):
         """Whole run on HOST float32 tensors (pinned for full PCIe speed); synchronises."""
+        n3 = 3 * self.n_particles
         for t in (h_pos, h_mom):
-            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
-                raise FpmError("nbody_host expects contiguous CPU float32 tensors")
-        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or t.numel() != n3:
+                raise FpmError("nbody_host expects contiguous CPU float32 [3][np^3] tensors")
+        st, n_steps = self._stages(stages)
         self._check(_lib.fpm_nbody_host(self._h, ctypes.c_void_p(h_pos.data_ptr()),
-                                        ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos), _dev(d_mom),
-                                        st, len(stages) - 1))
+                                        ctypes.c_void_p(h_mom.data_ptr()), _dev(d_pos, numel=n3, what="d_pos"),
+                                        _dev(d_mom, numel=n3, what="d_mom"), st, n_steps))
         return h_pos, h_mom
 
     def paint_adjoint(self, pos, grad_mesh, mass=None, want_grad_mass=True):
-        n = pos.shape[1]
+        n = _particles(pos)
         gpos = self._empty(3, n)
         gmass = self._empty(n) if want_grad_mass else None
-        self._check(_lib.fpm_paint_adjoint(self._h, _dev(pos), _dev(mass), n, _dev(grad_mesh),
-                                           _dev(gpos), _dev(gmass)))
+        self._check(_lib.fpm_paint_adjoint(self._h, _dev(pos), _dev(mass, numel=n, what="mass"), n,
+                                           _dev(grad_mesh, numel=self._n_g, what="grad_mesh"), _dev(gpos),
+                                           _dev(gmass)))
         return gpos, gmass
 
     def readout_adjoint(self, mesh, pos, grad_out, grad_mesh=None, want_grad_pos=True):
-        n = pos.shape[1]
+        n = _particles(pos)
         gm = grad_mesh if grad_mesh is not None else torch.zeros(self.ng, self.ng, self.ng,
                                                                   dtype=torch.float32, device=self.device)
         gpos = self._empty(3, n) if want_grad_pos else None
-        self._check(_lib.fpm_readout_adjoint(self._h, _dev(mesh), _dev(pos), n, _dev(grad_out),
-                                             _dev(gm), _dev(gpos)))
+        self._check(_lib.fpm_readout_adjoint(self._h, _dev(mesh, numel=self._n_g, what="mesh"), _dev(pos), n,
+                                             _dev(grad_out, numel=n, what="grad_out"),
+                                             _dev(gm, numel=self._n_g, what="grad_mesh"), _dev(gpos)))
         return gm, gpos
 
     # ---- reverse mode (SURVEY.md 8(c) R12) --------------------------------------------------
     def force_vjp(self, pos, v, coef=1.0, grad_pos=None):
         """grad_pos += coef * J_f(pos)^T v for f = force(pos); returns grad_pos [3][n]."""
-        n = pos.shape[1]
+        n = _particles(pos)
         g = grad_pos if grad_pos is not None else torch.zeros(3, n, dtype=torch.float32, device=self.device)
-        self._check(_lib.fpm_force_vjp(self._h, _dev(pos), n, _dev(v), float(coef), _dev(g)))
+        self._check(_lib.fpm_force_vjp(self._h, _dev(pos), n, _dev(v, numel=3 * n, what="v"), float(coef),
+                                       _dev(g, numel=3 * n, what="grad_pos")))
         return g
 
-    def nbody_vjp(self, traj, stages, grad_pos, grad_mom):
-        """Cotangents of the final (pos, mom) -> of the initial (pos, mom), in place."""
-        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
-        self._check(_lib.fpm_nbody_vjp(self._h, _dev(traj), st, len(stages) - 1, _dev(grad_pos),
-                                       _dev(grad_mom)))
+    def nbody_vjp(self, traj, stages, grad_pos, grad_mom, grad_mom_is_zero=False):
+        """Cotangents of the final (pos, mom) -> of the initial (pos, mom), in place.  grad_mom_is_zero: the
+        caller guarantees grad_mom holds zeros (loss on the final positions only): FPM_VJP_GRAD_MOM_ZERO."""
+        st, n_steps = self._stages(stages)
+        n3 = 3 * self.n_particles
+        self._check(_lib.fpm_nbody_vjp(self._h, _dev(traj, numel=(n_steps + 1) * n3, what="traj"), st, n_steps,
+                                       _dev(grad_pos, numel=n3, what="grad_pos"),
+                                       _dev(grad_mom, numel=n3, what="grad_mom"),
+                                       VJP_GRAD_MOM_ZERO if grad_mom_is_zero else 0))
         return grad_pos, grad_mom
 
     def lpt_init_vjp(self, delta_lin, a0, order, grad_pos, grad_mom):
         out = self._empty(self.np_side, self.np_side, self.np_side)
-        self._check(_lib.fpm_lpt_init_vjp(self._h, _dev(delta_lin), a0, order, _dev(grad_pos),
-                                          _dev(grad_mom), _dev(out)))
+        n3 = 3 * self.n_particles
+        self._check(_lib.fpm_lpt_init_vjp(self._h, _dev(delta_lin, numel=self.n_particles, what="delta_lin"), a0,
+                                          order, _dev(grad_pos, numel=n3, what="grad_pos"),
+                                          _dev(grad_mom, numel=n3, what="grad_mom"), _dev(out)))
         return out
 
     # ---- MAP reconstruction (SURVEY.md 8(f) N1; PAPER.md Eq. 12, Listing 7.1) -------------------
     def recon_loss_grad(self, s, data, sigma, inv_power, stages, lpt_order=2, scratch=None):
         """((likelihood term, prior term), gradient [np^3]) of the negative log-posterior of s."""
-        n_steps = len(stages) - 1
+        st, n_steps = self._stages(stages)
         need = _lib.fpm_recon_scratch_bytes(ctypes.byref(self._cfg), n_steps)
+        if scratch is None:
+            scratch = getattr(self, "_recon_scratch", None)      # reuse the one a previous call allocated
         if scratch is None or scratch.numel() * scratch.element_size() < need:
             scratch = torch.empty(need // 4, dtype=torch.float32, device=self.device)
-            self._recon_scratch = scratch
-        st = (ctypes.c_double * len(stages))(*[float(a) for a in stages])
+        self._recon_scratch = scratch
         grad = self._empty(self.np_side, self.np_side, self.np_side)
         loss = (ctypes.c_double * 2)()
-        self._check(_lib.fpm_recon_loss_grad(self._h, _dev(s), _dev(data), float(sigma), _dev(inv_power), st,
+        n_kp = self.np_side * self.np_side * (self.np_side // 2 + 1)
+        self._check(_lib.fpm_recon_loss_grad(self._h, _dev(s, numel=self.n_particles, what="s"),
+                                             _dev(data, numel=self._n_g, what="data"), float(sigma),
+                                             _dev(inv_power, numel=n_kp, what="inv_power"), st,
                                              n_steps, int(lpt_order), ctypes.c_void_p(scratch.data_ptr()),
                                              scratch.numel() * scratch.element_size(), _dev(grad), loss))
         return (loss[0], loss[1]), grad

@@ -62,9 +62,23 @@ int cuda_fail(fpm_ctx* ctx, cudaError_t e, const char* where) {
   return fail(ctx, FPM_ECUDA, buf);
 }
 
+// Every entry point runs on the device the context was created on, whatever device is current in the
+// calling thread; the caller's current device is restored on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 #define FPM_ENTER(ctx)                                              \
   if (!(ctx)) return FPM_EINVAL;                                    \
-  if ((ctx)->sticky) return FPM_ECUDA;
+  if ((ctx)->sticky) return FPM_ECUDA;                              \
+  DeviceGuard device_guard__((ctx)->device);
 #define FPM_CUDA(ctx, call)                                         \
   do {                                                              \
     cudaError_t e__ = (call);                                       \
@@ -173,6 +187,23 @@ int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, con
   return FPM_OK;
 }
 
+// merged kick / drift factors of the n_steps + 1 PM steps of a run (R6); see fpm_step_factors in fpm.h
+void step_factors(const fpm_ctx* ctx, const double* a, int n_steps, double* kf, double* dr) {
+  const double om = ctx->cfg.omega_m;
+  const int fm = ctx->cfg.factor_mode;
+  double pending = 0.0;   // second half kick of the previous step, same force mesh
+  for (int j = 0; j <= n_steps; ++j) {
+    kf[j] = pending;
+    dr[j] = 0.0;
+    if (j < n_steps) {
+      const double ai = a[j], af = a[j + 1], ah = std::sqrt(ai * af);
+      kf[j] += kick_factor(om, ai, ai, ah, fm);
+      dr[j] = drift_factor(om, ai, ah, af, fm);
+      pending = kick_factor(om, ah, af, af, fm);
+    }
+  }
+}
+
 }  // namespace
 
 extern "C" {
@@ -191,6 +222,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
   fpm_ctx* ctx = new (std::nothrow) fpm_ctx();
   if (!ctx) return FPM_ENOMEM;
   ctx->cfg = *cfg;
+  if (cudaGetDevice(&ctx->device) != cudaSuccess) { delete ctx; return FPM_ECUDA; }
   ctx->stream = static_cast<cudaStream_t>(cuda_stream);
   ctx->prof.stream = ctx->stream;
   cudaError_t e = fft_tables_create(cfg->ng, &ctx->fft_g);
@@ -208,6 +240,7 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
 
 int fpm_destroy(fpm_ctx* ctx) {
   if (!ctx) return FPM_EINVAL;
+  DeviceGuard device_guard__(ctx->device);
   ctx->prof.destroy();
   if (ctx->d_acc) cudaFree(ctx->d_acc);
   fft_tables_destroy(&ctx->fft_g);
@@ -253,6 +286,15 @@ int fpm_drift_factor(const fpm_ctx* ctx, double ai, double ac, double af, double
 int fpm_kick_factor(const fpm_ctx* ctx, double ai, double ac, double af, double* out) {
   if (!ctx || !out || !(ai > 0.0 && ac > 0.0 && af > 0.0)) return FPM_EINVAL;
   *out = kick_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
+  return FPM_OK;
+}
+
+int fpm_step_factors(const fpm_ctx* ctx, const double* a_stages, int n_steps, double* kick_fac,
+                     double* drift_fac) {
+  if (!ctx || !a_stages || !kick_fac || !drift_fac || n_steps < 0) return FPM_EINVAL;
+  for (int j = 0; j <= n_steps; ++j)
+    if (!(a_stages[j] > 0.0)) return FPM_EINVAL;
+  step_factors(ctx, a_stages, n_steps, kick_fac, drift_fac);
   return FPM_OK;
 }
 
@@ -406,22 +448,13 @@ int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int 
   cudaStream_t s = ctx->stream;
   const int np = ctx->cfg.np;
   const int64_t n = (int64_t)np * np * np;
-  const double om = ctx->cfg.omega_m;
-  const int fm = ctx->cfg.factor_mode;
-
-  double pending_kick = 0.0;   // second half kick of the previous step, same force mesh
+  std::vector<double> kf(n_steps + 1), dr(n_steps + 1);
+  step_factors(ctx, a_stages, n_steps, kf.data(), dr.data());
   for (int j = 0; j <= n_steps; ++j) {
     if (traj)
       FPM_CUDA(ctx, cudaMemcpyAsync(traj + (int64_t)j * 3 * n, pos, sizeof(float) * 3 * n,
                                     cudaMemcpyDeviceToDevice, s));
-    double kf = pending_kick, dr = 0.0;
-    if (j < n_steps) {
-      const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
-      kf += kick_factor(om, ai, ai, ah, fm);
-      dr = drift_factor(om, ai, ah, af, fm);
-      pending_kick = kick_factor(om, ah, af, af, fm);
-    }
-    const int rc = pm_step(ctx, w, pos, mom, n, kf, dr);
+    const int rc = pm_step(ctx, w, pos, mom, n, kf[j], dr[j]);
     if (rc != FPM_OK) return rc;
   }
   return FPM_OK;
@@ -478,29 +511,19 @@ int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, dou
 }
 
 int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n_steps,
-                  float* grad_pos, float* grad_mom) {
+                  float* grad_pos, float* grad_mom, int flags) {
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, traj && a_stages && grad_pos && grad_mom && n_steps >= 0, "fpm_nbody_vjp: bad arguments");
+  FPM_REQUIRE(ctx, (flags & ~FPM_VJP_GRAD_MOM_ZERO) == 0, "fpm_nbody_vjp: unknown flag");
   for (int j = 0; j <= n_steps; ++j)
     FPM_REQUIRE(ctx, a_stages[j] > 0.0, "fpm_nbody_vjp: scale factors must be positive");
   FPM_NEED_WS(ctx);
   const Workspace w = carve(ctx);
   const int np = ctx->cfg.np;
   const int64_t n = (int64_t)np * np * np;
-  const double om = ctx->cfg.omega_m;
-  const int fm = ctx->cfg.factor_mode;
   // the same merged factors as fpm_nbody: step j is  p += kf_j f(x_j);  x = wrap(x + dr_j p)
   std::vector<double> kf(n_steps + 1), dr(n_steps + 1);
-  double pending = 0.0;
-  for (int j = 0; j <= n_steps; ++j) {
-    kf[j] = pending; dr[j] = 0.0;
-    if (j < n_steps) {
-      const double ai = a_stages[j], af = a_stages[j + 1], ah = std::sqrt(ai * af);
-      kf[j] += kick_factor(om, ai, ai, ah, fm);
-      dr[j] = drift_factor(om, ai, ah, af, fm);
-      pending = kick_factor(om, ah, af, af, fm);
-    }
-  }
+  step_factors(ctx, a_stages, n_steps, kf.data(), dr.data());
   for (int j = n_steps; j >= 0; --j) {
     // x' = wrap(x + dr p'):  p'_bar += dr x'_bar   (wrap has unit derivative)
     if (dr[j] != 0.0) {
@@ -508,6 +531,8 @@ int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n
       FPM_CUDA(ctx, axpy(grad_mom, grad_pos, (float)dr[j], 3 * n, ctx->stream));
     }
     // p' = p + kf f(x_j):  x_bar += kf J_f(x_j)^T p'_bar
+    // (with a loss on the final positions only, p'_bar of the last step is identically zero: nothing to add)
+    if (j == n_steps && (flags & FPM_VJP_GRAD_MOM_ZERO)) continue;
     if (kf[j] != 0.0) {
       const int rc = force_vjp(ctx, w, traj + (int64_t)j * 3 * n, n, grad_mom, kf[j], grad_pos);
       if (rc != FPM_OK) return rc;
@@ -623,7 +648,7 @@ int fpm_recon_loss_grad(fpm_ctx* ctx, const float* s_lin, const float* data, dou
   { ProfScope sc(pr, K_READOUT_GRAD);
     FPM_CUDA(ctx, readout_grad(w.F[0], pos, nullptr, particle_mass(ctx), n, ng, gx, nullptr, st)); }
   FPM_CUDA(ctx, cudaMemsetAsync(gp, 0, sizeof(float) * 3 * n, st));
-  rc = fpm_nbody_vjp(ctx, traj, a_stages, n_steps, gx, gp);
+  rc = fpm_nbody_vjp(ctx, traj, a_stages, n_steps, gx, gp, FPM_VJP_GRAD_MOM_ZERO);
   if (rc != FPM_OK) return rc;
   rc = fpm_lpt_init_vjp(ctx, s_lin, a_stages[0], lpt_order, gx, gp, grad);
   if (rc != FPM_OK) return rc;
@@ -656,6 +681,7 @@ int fpm_adam_step(fpm_ctx* ctx, float* x, const float* grad, float* m, float* v,
 
 int fpm_profile_enable(fpm_ctx* ctx, int on) {
   if (!ctx) return FPM_EINVAL;
+  DeviceGuard device_guard__(ctx->device);
   ctx->prof.flush();
   ctx->prof.enabled = on != 0;
   return FPM_OK;
@@ -663,12 +689,14 @@ int fpm_profile_enable(fpm_ctx* ctx, int on) {
 
 int fpm_profile_reset(fpm_ctx* ctx) {
   if (!ctx) return FPM_EINVAL;
+  DeviceGuard device_guard__(ctx->device);
   ctx->prof.reset();
   return FPM_OK;
 }
 
 int fpm_profile_read(fpm_ctx* ctx, int kernel_id, const char** name, double* total_ms, int64_t* count) {
   if (!ctx || kernel_id < 0 || kernel_id >= K_COUNT) return FPM_EINVAL;
+  DeviceGuard device_guard__(ctx->device);
   ctx->prof.flush();
   if (name) *name = kernel_name(kernel_id);
   if (total_ms) *total_ms = ctx->prof.ms[kernel_id];

@@ -48,10 +48,7 @@ void build_stage_table(const PlanInfo& pi, std::vector<float2>& out) {
 }
 
 template <class K>
-cudaError_t set_smem(K kernel, size_t bytes) {
-  if (bytes <= 48 * 1024) return cudaSuccess;
-  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-}
+cudaError_t set_smem(K kernel, size_t bytes) { return ensure_dynamic_smem(kernel, bytes); }
 
 template <int N, bool INV>
 cudaError_t launch_cols(const float2* in, float2* out, int batches, int64_t batch_stride, int ncols,

@@ -41,6 +41,21 @@ struct ProfScope {
   ~ProfScope() { if (p) p->end(); }
 };
 
+// Opt a kernel in to more than 48 KB of dynamic shared memory, once per kernel and device (the attribute
+// is per device; calling cudaFuncSetAttribute before every launch showed up on the small configurations).
+template <class K>
+inline cudaError_t ensure_dynamic_smem(K kernel, size_t bytes) {
+  if (bytes <= 48 * 1024) return cudaSuccess;
+  static bool done[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess && dev >= 0 && dev < 64) done[dev] = true;
+  return e;
+}
+
 // ---- FFT (fft.cu) ---------------------------------------------------------------------------
 struct FftTables {
   int n = 0;
@@ -168,6 +183,7 @@ double kick_factor(double omega_m, double ai, double ac, double af, int factor_m
 
 struct fpm_ctx {
   fpm_config cfg;
+  int device = 0;                   // the CUDA device that was current in fpm_create; every call runs there
   cudaStream_t stream = nullptr;
   fpm::FftTables fft_g, fft_p;      // plans for ng and np (same object when equal)
   fpm::KernelTables kt_g, kt_p;     // transfer-function tables on ng; spectral tables on np

@@ -15,6 +15,9 @@
 //     (RED.E.ADD.F32x4); the few particles outside the window fall back to direct reductions.
 //     Shared memory has no native fp32 add (ATOMS.CAST.SPIN loop), so the window accumulates in
 //     32-bit fixed point with a per-brick scale that cannot overflow (native ATOMS.ADD).
+#include <cstdlib>
+#include <type_traits>
+
 #include "fpm_internal.h"
 
 namespace fpm {
@@ -41,18 +44,10 @@ __device__ __forceinline__ float fast_floor(float x, int& i) {
   if (r > x) { r -= 1.f; i -= 1; }
   return r;
 }
-__device__ __forceinline__ int fast_round_to_int(float x) { return __float_as_int(x + kMagic) - kMagicBits; }
 // round(a * b) with one rounding: the product is formed inside the FMA that adds the magic constant
 __device__ __forceinline__ int fast_round_mul_to_int(float a, float b) {
   return __float_as_int(fmaf(a, b, kMagic)) - kMagicBits;
 }
-// CIC split without compare/select: i = rint(x - 1/2), t = x - i.  Equal to (floor(x), x - floor(x)) unless
-// x is an integer k, where it may give (k - 1, 1) instead of (k, 0): the same deposit (weight 1 on cell k).
-__device__ __forceinline__ float cic_split(float x, int& i) {
-  const float r = fast_rint(x - 0.5f, i);
-  return x - r;
-}
-
 __device__ __forceinline__ Cic cic_of(float x, float y, float z, int mask) {
   Cic c;
   const float p[3] = {x, y, z};
@@ -90,7 +85,7 @@ constexpr int kBrickThreads = 512;
 constexpr int kPerThread = kBrick / kBrickThreads;
 
 struct BrickMap {
-  int np, nbz, nby;
+  int np, nbz, nby, lg_np;
   __device__ __forceinline__ void origin(int64_t bid, int& qx0, int& qy0, int& qz0) const {
     const int bz = (int)(bid % nbz);
     const int64_t r = bid / nbz;
@@ -148,139 +143,202 @@ constexpr int WX = BX + 2 * kHalo + 1, WY = BY + 2 * kHalo + 1;
 constexpr int WZ = (BZ + 2 * kHalo + 1 + 3 + 3) & ~3;
 constexpr int kWinCells = WX * WY * WZ;       // 13 x 21 x 40 = 10920 cells, 43.7 KB
 
+// floor without the conversion pipe: a round-down add of 1.5 * 2^23 leaves floor(x) in the low mantissa
+// bits (exact for |x| < 2^22).  Returns floor(x) as a float; bits = kMagicBits + floor(x).
+__device__ __forceinline__ float floor_magic(float x, int& bits) {
+  const float t = __fadd_rd(x, kMagic);
+  bits = __float_as_int(t);
+  return t - kMagic;
+}
+
+// shared-memory reductions at [addr + OFF] with the offset folded into the instruction (ATOMS.ADD with an
+// immediate): one base register serves the 8 corners of a particle
+template <int OFF>
+__device__ __forceinline__ void red_shared(unsigned addr, int v) {
+  asm volatile("red.shared.add.u32 [%0+%2], %1;" ::"r"(addr), "r"(v), "n"(OFF) : "memory");
+}
+template <int OFF>
+__device__ __forceinline__ void red_shared(unsigned addr, float v) {
+  asm volatile("red.shared.add.f32 [%0+%2], %1;" ::"r"(addr), "f"(v), "n"(OFF) : "memory");
+}
+// the four cells (y, y+1) x (z, z+1) of one x plane of the window
+template <int OFF, class V>
+__device__ __forceinline__ void red_plane(unsigned addr, const V (&v)[4]) {
+  red_shared<OFF>(addr, v[0]);
+  red_shared<OFF + 4>(addr, v[1]);
+  red_shared<OFF + 4 * WZ>(addr, v[2]);
+  red_shared<OFF + 4 * WZ + 4>(addr, v[3]);
+}
+
 // RES = ng / np (1 or 2): the lattice spacing in cells.  The CTA's sub-brick of (8 x 16 x 32) / RES lattice
 // sites always spans 8 x 16 x 32 cells, so the window is the same; with RES = 2 a thread owns one particle.
-template <bool FIXED, bool HAS_MASS, int RES = 1>
+//
+// FIXED: the window accumulates round(m w s) as 32-bit integers (native ATOMS.ADD), s a per-brick power of
+// two:  s = 2^floor(log2 min(2^30 / sum_p |m_p|, 2^21 / max_p |m_p|))  (2^31 when every mass is the same
+// positive constant: all deposits are >= 0 and the window is read back as unsigned).  No cell can overflow:
+// a particle gives a cell at most its whole mass, so |cell| <= s sum|m| + particles/2 < 2^31 (resp. 2^32);
+// the magic-number rounding needs |m w s| < 2^22.  Error per deposit <= 1/(2 s): 2^-20 m for the density
+// paint of a run, <= max(2^-19 mean|m|, 2^-22 max|m|) with per-particle masses.  A brick whose masses are
+// badly conditioned for that (max|m| > 64 mean|m|) or not finite is deposited with plain fp32 reductions
+// instead, so an outlier or a NaN/Inf behaves as it would in the direct kernel.
+// XMERGE (RES = 1): a thread's 8 particles are neighbours along x; when particle k+1 falls in the next x
+// plane of the same (y, z) cell column, its lower-plane deposits are added in registers to the upper-plane
+// deposits of particle k and go out as 4 reductions instead of 8.
+template <bool FIXED, bool HAS_MASS, int RES = 1, bool XMERGE = false>
 __global__ void __launch_bounds__(kBrickThreads, 2)
 paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
                    int64_t n, BrickMap bm, int ng, float* __restrict__ mesh) {
   constexpr int SX = BX / RES, SY = BY / RES, SZ = BZ / RES;          // lattice sites of the sub-brick
   constexpr int kPerThread = SX * SY * SZ / kBrickThreads;
+  constexpr int kPerCta = SX * SY * SZ;
   static_assert(kPerThread >= 1 && SX % kPerThread == 0, "sub-brick shape");
+  static_assert(!XMERGE || (RES == 1 && FIXED), "x-merge is implemented for the fixed-point lattice walk");
+  using V = typename std::conditional<FIXED, int, float>::type;
   extern __shared__ __align__(16) float win_f[];
-  int* win_i = reinterpret_cast<int*>(win_f);
-  __shared__ float red[4][kBrickThreads / 32];
+  __shared__ int red_i[3][kBrickThreads / 32];
+  __shared__ float red_f[2][kBrickThreads / 32];
   const int mask = ng - 1;
-  const float fng = (float)ng, inv_ng = 1.f / fng;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  // sub-brick origin (lattice sites) and this thread's first site: slot s = tid + 512 k has offsets
-  // lz = s % SZ, ly = (s / SZ) % SY, lx = s / (SZ SY)  (RES = 1: lz = lane, ly = warp, lx = k)
-  const int nbz = bm.np / SZ, nby = bm.np / SY;
-  const int qz0 = (int)(blockIdx.x % nbz) * SZ, qy0 = (int)((blockIdx.x / nbz) % nby) * SY,
-            qx0 = (int)(blockIdx.x / nbz / nby) * SX;
+  // sub-brick origin (lattice sites): np is a power of two, so the brick coordinates are bit fields
+  const int lg_nbz = bm.lg_np - (RES == 1 ? 5 : 4), lg_nby = bm.lg_np - (RES == 1 ? 4 : 3);
+  const unsigned bid = blockIdx.x;
+  const int qz0 = (int)(bid & ((1u << lg_nbz) - 1)) * SZ, qy0 = (int)((bid >> lg_nbz) & ((1u << lg_nby) - 1)) * SY,
+            qx0 = (int)(bid >> (lg_nbz + lg_nby)) * SX;
   const int lz = tid % SZ, ly = (tid / SZ) % SY, lx0 = tid / (SZ * SY);
   constexpr int kDx = kBrickThreads / (SZ * SY);     // lattice planes advanced per k
-
-  for (int i = tid; i < kWinCells / 4; i += kBrickThreads)
-    reinterpret_cast<float4*>(win_f)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
   float x[kPerThread], y[kPerThread], z[kPerThread], m[HAS_MASS ? kPerThread : 1];
   const int64_t plane = (int64_t)bm.np * bm.np;
   const int64_t p0 = ((int64_t)(qx0 + lx0) * bm.np + (qy0 + ly)) * bm.np + (qz0 + lz);
+  const float *px = pos + p0, *py = px + n, *pz = py + n;
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
-    const int64_t p = p0 + (int64_t)(k * kDx) * plane;
-    x[k] = ld_stream(pos + p);
-    y[k] = ld_stream(pos + n + p);
-    z[k] = ld_stream(pos + 2 * n + p);
-    if (HAS_MASS) m[k] = ld_stream(mass + p);
+    const int64_t o = (int64_t)(k * kDx) * plane;
+    x[k] = ld_stream(px + o);
+    y[k] = ld_stream(py + o);
+    z[k] = ld_stream(pz + o);
+    if (HAS_MASS) m[k] = ld_stream(mass + p0 + o);
   }
-  // mean displacement from the lattice sites (wrapped to [-ng/2, ng/2)) places the window
-  float sx = 0.f, sy = 0.f, sz = 0.f, mmax = HAS_MASS ? 0.f : fabsf(mass_const);
-  const float qy = (float)((qy0 + ly) * RES), qz = (float)((qz0 + lz) * RES);    // lattice site in cells
-  // (a sample of kMeanPlanes of the brick's x planes is enough: the window position only decides how
-  //  many particles take the slow path, never the result)
-  constexpr int kMeanPlanes = kPerThread >= 2 ? 2 : 1, kMeanStep = kPerThread / kMeanPlanes;
-#pragma unroll
-  for (int k = 0; k < kPerThread; ++k) {
-    if (k % kMeanStep == 0) {
-      float dx = x[k] - (float)((qx0 + lx0 + k * kDx) * RES), dy = y[k] - qy, dz = z[k] - qz;
-      int unused;
-      dx -= fng * fast_rint(dx * inv_ng, unused);
-      dy -= fng * fast_rint(dy * inv_ng, unused);
-      dz -= fng * fast_rint(dz * inv_ng, unused);
-      sx += dx; sy += dy; sz += dz;
-    }
-    if (HAS_MASS) mmax = fmaxf(mmax, fabsf(m[k]));
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    sx += __shfl_xor_sync(0xffffffffu, sx, o);
-    sy += __shfl_xor_sync(0xffffffffu, sy, o);
-    sz += __shfl_xor_sync(0xffffffffu, sz, o);
-    if (HAS_MASS) mmax = fmaxf(mmax, __shfl_xor_sync(0xffffffffu, mmax, o));
-  }
-  if (lane == 0) { red[0][warp] = sx; red[1][warp] = sy; red[2][warp] = sz; red[3][warp] = mmax; }
-  __syncthreads();   // also orders the window zeroing before the deposits
-  sx = sy = sz = 0.f;
-#pragma unroll
-  for (int i = 0; i < kBrickThreads / 32; ++i) {
-    sx += red[0][i]; sy += red[1][i]; sz += red[2][i];
-    if (HAS_MASS) mmax = fmaxf(mmax, red[3][i]);
-  }
-  constexpr float inv_cnt = 1.f / (float)(kBrickThreads * kMeanPlanes);
-  int mx, my, mz;
-  fast_floor(sx * inv_cnt, mx);
-  fast_floor(sy * inv_cnt, my);
-  fast_floor(sz * inv_cnt, mz);
-  const int ox = qx0 * RES + mx - kHalo;
-  const int oy = qy0 * RES + my - kHalo;
-  const int oz = (qz0 * RES + mz - kHalo) & ~3;
-  // Fixed point with a power-of-two scale 2^floor(log2(2^18 / mmax)) (exact for weights that are dyadic
-  // fractions).  No cell can overflow: |sum of the brick's deposits| <= kBrick (mmax scale + 1/2)
-  // <= 2^30 + 2^11 < 2^31.  With one positive mass for all particles (the density paint of a run) every
-  // deposit is >= 0, the window is read back as unsigned and the scale is 2^19: sums < 2^31 + 2^11 < 2^32.
-  // (in general 2^30 resp. 2^31 over the particles per CTA, capped at 2^21: the magic-number rounding
-  // needs |deposit| < 2^22; a RES = 2 sub-brick holds 512 particles and reaches the cap)
-  const bool nonneg = !HAS_MASS && mass_const > 0.f;
-  constexpr int kPerCta = SX * SY * SZ;
-  constexpr float kTopSigned = (float)((1 << 30) / kPerCta < (1 << 21) ? (1 << 30) / kPerCta : (1 << 21));
-  constexpr float kTopUnsigned = 2.f * kTopSigned < (float)(1 << 21) ? 2.f * kTopSigned : (float)(1 << 21);
-  const float top = nonneg ? kTopUnsigned : kTopSigned;
-  const float scale = FIXED ? (mmax > 0.f ? __int_as_float(__float_as_int(top / mmax) & 0x7F800000) : 0.f) : 1.f;
+  for (int i = tid; i < kWinCells / 4; i += kBrickThreads)
+    reinterpret_cast<float4*>(win_f)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
+  // Window placement: mean cell displacement floor(x) - site (wrapped to [-ng/2, ng/2)) over a sample of the
+  // brick's x planes, in integers (order-independent, so every thread gets the same origin).  The position
+  // only decides how many particles take the slow path, never the result.
+  constexpr int kMeanPlanes = kPerThread >= 2 ? 2 : 1, kMeanStep = kPerThread / kMeanPlanes;
+  constexpr int kLgCnt = (RES == 1 ? 10 : 9);        // log2(kBrickThreads * kMeanPlanes)
+  static_assert((1 << kLgCnt) == kBrickThreads * kMeanPlanes, "mean sample count");
+  int sx = 0, sy = 0, sz = 0;
+  const int half = ng >> 1;
+#pragma unroll
+  for (int k = 0; k < kPerThread; k += kMeanStep) {
+    int bx, by, bz;
+    floor_magic(x[k], bx); floor_magic(y[k], by); floor_magic(z[k], bz);
+    sx += ((bx - kMagicBits - (qx0 + lx0 + k * kDx) * RES + half) & mask) - half;
+    sy += ((by - kMagicBits - (qy0 + ly) * RES + half) & mask) - half;
+    sz += ((bz - kMagicBits - (qz0 + lz) * RES + half) & mask) - half;
+  }
+  sx = __reduce_add_sync(0xffffffffu, sx);
+  sy = __reduce_add_sync(0xffffffffu, sy);
+  sz = __reduce_add_sync(0xffffffffu, sz);
+  float sumabs = 0.f;
+  unsigned mmax_bits = 0;
+  if (HAS_MASS) {
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      sumabs += fabsf(m[k]);
+      mmax_bits = max(mmax_bits, (unsigned)__float_as_int(fabsf(m[k])));   // |m| as bits: NaN > Inf > finite
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sumabs += __shfl_xor_sync(0xffffffffu, sumabs, o);
+    mmax_bits = __reduce_max_sync(0xffffffffu, mmax_bits);
+  }
+  if (lane == 0) {
+    red_i[0][warp] = sx; red_i[1][warp] = sy; red_i[2][warp] = sz;
+    if (HAS_MASS) { red_f[0][warp] = sumabs; red_f[1][warp] = __uint_as_float(mmax_bits); }
+  }
+  __syncthreads();   // also orders the window zeroing before the deposits
+  constexpr int kWarps = kBrickThreads / 32;
+  sx = __reduce_add_sync(0xffffffffu, lane < kWarps ? red_i[0][lane] : 0);
+  sy = __reduce_add_sync(0xffffffffu, lane < kWarps ? red_i[1][lane] : 0);
+  sz = __reduce_add_sync(0xffffffffu, lane < kWarps ? red_i[2][lane] : 0);
+  // mean displacement = mean(floor) + 1/2 on average; the window is centred on floor(mean)
+  const int ox = qx0 * RES + ((sx + (1 << (kLgCnt - 1))) >> kLgCnt) - kHalo;
+  const int oy = qy0 * RES + ((sy + (1 << (kLgCnt - 1))) >> kLgCnt) - kHalo;
+  const int oz = (qz0 * RES + ((sz + (1 << (kLgCnt - 1))) >> kLgCnt) - kHalo) & ~3;
+  float mmax = fabsf(mass_const);
+  sumabs = (float)kPerCta * mmax;
+  bool use_window = true;
+  if (HAS_MASS) {
+    sumabs = lane < kWarps ? red_f[0][lane] : 0.f;
+    mmax_bits = lane < kWarps ? (unsigned)__float_as_int(red_f[1][lane]) : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sumabs += __shfl_xor_sync(0xffffffffu, sumabs, o);
+    mmax_bits = __reduce_max_sync(0xffffffffu, mmax_bits);
+    mmax = __uint_as_float(mmax_bits);
+    // fixed point only for a finite, reasonably conditioned brick (see the kernel comment)
+    if (FIXED) use_window = mmax_bits < 0x7F800000u && sumabs < 3.0e38f && mmax * (float)kPerCta <= 64.f * sumabs;
+  }
+  const bool nonneg = !HAS_MASS && mass_const > 0.f;
+  float scale = 1.f;
+  if (FIXED) {
+    const float cap = fminf((nonneg ? 2147483648.f : 1073741824.f) / sumabs, 2097152.f / mmax);
+    scale = (mmax > 0.f && use_window) ? __int_as_float(__float_as_int(cap) & 0x7F800000) : 0.f;
+  }
+  const unsigned win_s = (unsigned)__cvta_generic_to_shared(win_f);
+  const int cx = -kMagicBits - ox, cy = -kMagicBits - oy, cz = -kMagicBits - oz;
+
+  unsigned pend = 0xffffffffu;     // XMERGE: window address of the deposits waiting in pv
+  V pv[4] = {};
 #pragma unroll
   for (int k = 0; k < kPerThread; ++k) {
-    int ix, iy, iz;
-    const float tx = cic_split(x[k], ix), ty = cic_split(y[k], iy), tz = cic_split(z[k], iz);
-    const unsigned rx = (ix - ox) & mask, ry = (iy - oy) & mask, rz = (iz - oz) & mask;
+    int bx, by, bz;
+    const float tx = x[k] - floor_magic(x[k], bx), ty = y[k] - floor_magic(y[k], by),
+                tz = z[k] - floor_magic(z[k], bz);
+    const unsigned rx = (bx + cx) & mask, ry = (by + cy) & mask, rz = (bz + cz) & mask;
     const float mk = HAS_MASS ? m[k] : mass_const;
-    if (rx < WX - 1 && ry < WY - 1 && rz < WZ - 1) {
+    if (rx < WX - 1 && ry < WY - 1 && rz < WZ - 1 && use_window) {
       const float mm = mk * scale;
-      const float w00 = mm * (1.f - tx) * (1.f - ty), w01 = mm * (1.f - tx) * ty;
-      const float w10 = mm * tx * (1.f - ty), w11 = mm * tx * ty;
-      const float wz0 = 1.f - tz, wz1 = tz;
-      const int base = (rx * WY + ry) * WZ + rz;
+      const float m0 = mm - mm * tx, m1 = mm * tx;                 // mass in x planes ix, ix + 1
+      const float w00 = m0 - m0 * ty, w01 = m0 * ty, w10 = m1 - m1 * ty, w11 = m1 * ty;
+      const float wz0 = 1.f - tz;
+      const unsigned addr = win_s + 4u * ((rx * WY + ry) * WZ + rz);
+      V lo[4], hi[4];
       if (FIXED) {
-        int* c = win_i + base;
-        atomicAdd(c, fast_round_mul_to_int(w00, wz0));
-        atomicAdd(c + 1, fast_round_mul_to_int(w00, wz1));
-        atomicAdd(c + WZ, fast_round_mul_to_int(w01, wz0));
-        atomicAdd(c + WZ + 1, fast_round_mul_to_int(w01, wz1));
-        atomicAdd(c + WY * WZ, fast_round_mul_to_int(w10, wz0));
-        atomicAdd(c + WY * WZ + 1, fast_round_mul_to_int(w10, wz1));
-        atomicAdd(c + WY * WZ + WZ, fast_round_mul_to_int(w11, wz0));
-        atomicAdd(c + WY * WZ + WZ + 1, fast_round_mul_to_int(w11, wz1));
+        lo[0] = fast_round_mul_to_int(w00, wz0); lo[1] = fast_round_mul_to_int(w00, tz);
+        lo[2] = fast_round_mul_to_int(w01, wz0); lo[3] = fast_round_mul_to_int(w01, tz);
+        hi[0] = fast_round_mul_to_int(w10, wz0); hi[1] = fast_round_mul_to_int(w10, tz);
+        hi[2] = fast_round_mul_to_int(w11, wz0); hi[3] = fast_round_mul_to_int(w11, tz);
       } else {
-        float* c = win_f + base;
-        atomicAdd(c, w00 * wz0);
-        atomicAdd(c + 1, w00 * wz1);
-        atomicAdd(c + WZ, w01 * wz0);
-        atomicAdd(c + WZ + 1, w01 * wz1);
-        atomicAdd(c + WY * WZ, w10 * wz0);
-        atomicAdd(c + WY * WZ + 1, w10 * wz1);
-        atomicAdd(c + WY * WZ + WZ, w11 * wz0);
-        atomicAdd(c + WY * WZ + WZ + 1, w11 * wz1);
+        lo[0] = w00 * wz0; lo[1] = w00 * tz; lo[2] = w01 * wz0; lo[3] = w01 * tz;
+        hi[0] = w10 * wz0; hi[1] = w10 * tz; hi[2] = w11 * wz0; hi[3] = w11 * tz;
+      }
+      if (XMERGE) {
+        if (addr == pend) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) lo[j] += pv[j];
+        } else if (pend != 0xffffffffu) {
+          red_plane<0>(pend, pv);
+        }
+        red_plane<0>(addr, lo);
+        pend = addr + 4u * WY * WZ;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) pv[j] = hi[j];
+      } else {
+        red_plane<0>(addr, lo);
+        red_plane<4 * WY * WZ>(addr, hi);
       }
     } else {
       Cic c;
       c.t[0] = tx; c.t[1] = ty; c.t[2] = tz;
+      const int ix = bx - kMagicBits, iy = by - kMagicBits, iz = bz - kMagicBits;
       c.i0[0] = ix & mask; c.i1[0] = (ix + 1) & mask;
       c.i0[1] = iy & mask; c.i1[1] = (iy + 1) & mask;
       c.i0[2] = iz & mask; c.i1[2] = (iz + 1) & mask;
       deposit_global(mesh, ng, c, mk);
     }
   }
+  if (XMERGE && pend != 0xffffffffu) red_plane<0>(pend, pv);
   __syncthreads();
 
   // flush: one 16-byte vector reduction per 4 z-cells (oz and ng are multiples of 4)
@@ -290,22 +348,19 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   constexpr int dKz = kBrickThreads % WZ4, dRow = kBrickThreads / WZ4, dKy = dRow % WY, dKx = dRow / WY;
   static_assert(dKy + 1 < WY, "one carry per step");
   int kz = tid % WZ4, ky = (tid / WZ4) % WY, kx = (tid / WZ4) / WY;
+  const int* win_i = reinterpret_cast<const int*>(win_f);
   for (int gidx = tid; gidx < kWinCells / 4; gidx += kBrickThreads) {
-    float4 v;
-    bool any;
-    if (FIXED) {
-      const int4 q = reinterpret_cast<const int4*>(win_i)[gidx];
-      any = (q.x | q.y | q.z | q.w) != 0;
-      if (nonneg)
+    const int4 q = reinterpret_cast<const int4*>(win_i)[gidx];
+    // (an all-zero group holds no deposit, in fixed point and -- as +0.0f bit patterns or -0.0f -- in fp32)
+    if (((q.x | q.y | q.z | q.w) & (FIXED ? -1 : 0x7fffffff)) != 0) {
+      float4 v;
+      if (!FIXED)
+        v = make_float4(__int_as_float(q.x), __int_as_float(q.y), __int_as_float(q.z), __int_as_float(q.w));
+      else if (nonneg)
         v = make_float4(__uint2float_rn((unsigned)q.x) * inv_scale, __uint2float_rn((unsigned)q.y) * inv_scale,
                         __uint2float_rn((unsigned)q.z) * inv_scale, __uint2float_rn((unsigned)q.w) * inv_scale);
       else
         v = make_float4(q.x * inv_scale, q.y * inv_scale, q.z * inv_scale, q.w * inv_scale);
-    } else {
-      v = reinterpret_cast<const float4*>(win_f)[gidx];
-      any = !(v.x == 0.f && v.y == 0.f && v.z == 0.f && v.w == 0.f);
-    }
-    if (any) {
       const unsigned gx = (ox + kx) & mask, gy = (oy + ky) & mask, gz = (oz + 4 * kz) & mask;
       atomicAdd(reinterpret_cast<float4*>(mesh + ((gx * (unsigned)ng + gy) * (unsigned)ng + gz)), v);
     }
@@ -704,7 +759,8 @@ inline bool aligned16(const void* a, const void* b = nullptr, const void* c = nu
 
 inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kThreads - 1) / kThreads); }
 
-inline BrickMap brick_map(int np) { return BrickMap{np, np / BZ, np / BY}; }
+inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+inline BrickMap brick_map(int np) { return BrickMap{np, np / BZ, np / BY, ilog2(np)}; }
 
 }  // namespace
 
@@ -729,7 +785,7 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
   const unsigned grid = (unsigned)(n / (kBrick / (res * res * res)));
   const BrickMap bm = brick_map(ord.np);
   auto go = [&](auto kern) -> cudaError_t {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = ensure_dynamic_smem(kern, smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kBrickThreads, smem, s>>>(pos, mass, mass_const, n, bm, ng, mesh);
     return cudaGetLastError();
@@ -739,8 +795,11 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
       return mass ? go(paint_brick_kernel<true, true, 2>) : go(paint_brick_kernel<true, false, 2>);
     return mass ? go(paint_brick_kernel<false, true, 2>) : go(paint_brick_kernel<false, false, 2>);
   }
-  if (mode == FPM_PAINT_BRICK_FIXED)
+  if (mode == FPM_PAINT_BRICK_FIXED) {
+    static const bool xmerge = !(std::getenv("FPM_TUNE_XMERGE") && std::getenv("FPM_TUNE_XMERGE")[0] == '0');
+    if (xmerge) return mass ? go(paint_brick_kernel<true, true, 1, true>) : go(paint_brick_kernel<true, false, 1, true>);
     return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
+  }
   return mass ? go(paint_brick_kernel<false, true>) : go(paint_brick_kernel<false, false>);
 }
 
@@ -752,7 +811,7 @@ cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, floa
                                                                            brick_map(ord.np), out);
   else
     readout_kernel<1, false><<<blocks_for(n), kThreads, 0, s>>>(mesh, nullptr, nullptr, pos, n, ng,
-                                                               BrickMap{0, 1, 1}, out);
+                                                               BrickMap{0, 1, 1, 0}, out);
   return cudaGetLastError();
 }
 
@@ -763,7 +822,7 @@ cudaError_t readout3(const float* fx, const float* fy, const float* fz, const fl
     readout_kernel<3, true><<<(unsigned)(n / kBrick), kBrickThreads, 0, s>>>(fx, fy, fz, pos, n, ng,
                                                                            brick_map(ord.np), out3);
   else
-    readout_kernel<3, false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, n, ng, BrickMap{0, 1, 1}, out3);
+    readout_kernel<3, false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, n, ng, BrickMap{0, 1, 1, 0}, out3);
   return cudaGetLastError();
 }
 

@@ -11,6 +11,28 @@ def env_world():
             int(os.environ.get("WORLD_SIZE", "1")))
 
 
+def needs_spawn(n_gpus):
+    """True when N > 1 replicas were asked for but this process was not started by torchrun: the caller must
+    start the N ranks itself (launch_command) instead of quietly running one."""
+    return int(n_gpus) > 1 and "WORLD_SIZE" not in os.environ
+
+
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_command(n_gpus, script, argv, port=None, python=None):
+    """The torchrun command line that runs `script argv` as n_gpus replica ranks on this node (one process
+    per GPU, rendezvous on 127.0.0.1) -- the same launch the bench contract describes for N > 1."""
+    import sys
+    return [python or sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+            f"--nproc-per-node={int(n_gpus)}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port if port is not None else free_port()), script] + list(argv)
+
+
 def replica_seed(base_seed, rank):
     """Seed of the white-noise field of the replica on `rank`: distinct simulations, same cosmology."""
     return int(base_seed) + int(rank)

@@ -57,7 +57,8 @@ def test_argument_validation_needs_no_gpu():
     assert lib.fpm_recon_scratch_bytes(ctypes.byref(good), -1) == 0
     assert lib.fpm_recon_scratch_bytes(ctypes.byref(Cfg(500, 500, 0.3, 0, 0, 0, 0, 0)), 5) == 0
     assert lib.fpm_force_vjp(None, None, ctypes.c_int64(0), None, ctypes.c_double(1.0), None) == -1
-    assert lib.fpm_nbody_vjp(None, None, None, 0, None, None) == -1
+    assert lib.fpm_nbody_vjp(None, None, None, 0, None, None, 0) == -1
+    assert lib.fpm_step_factors(None, None, 0, None, None) == -1
     assert lib.fpm_lpt_init_vjp(None, None, ctypes.c_double(0.1), 2, None, None, None) == -1
     assert lib.fpm_adam_step(None, None, None, None, None, ctypes.c_int64(0), ctypes.c_double(0.1),
                              ctypes.c_double(0.9), ctypes.c_double(0.999), ctypes.c_double(1e-8), 1) == -1

@@ -76,6 +76,49 @@ def test_nbody_vjp_matches_oracle(fpm, oracle, np_side, ng, n_steps, force_path)
     assert rel_l2(host(dgp), rgp) < TOL
 
 
+def test_nbody_vjp_grad_mom_zero_flag_changes_nothing(fpm):
+    """FPM_VJP_GRAD_MOM_ZERO skips the last force VJP, which adds kf * J^T 0 = 0 when grad_mom enters as zeros."""
+    import torch
+    cfg = fi.Config("T", 32, 32, 100.0, 2, 3)
+    ctx = fpm.FPM(32, 32, box=cfg.box, force_path=1)
+    pos, mom = ctx.lpt_init(dev(fi.linear_field(32, cfg.box, 2)), cfg.a0, 2)
+    n, stages = 32 ** 3, cfg.stages()
+    traj = torch.empty(4, 3, n, device="cuda")
+    ctx.nbody(pos, mom, stages, traj=traj)
+    gx = np.random.default_rng(5).standard_normal((3, n)).astype(np.float32)
+    a_gx, a_gp = dev(gx), torch.zeros(3, n, device="cuda")
+    b_gx, b_gp = dev(gx), torch.zeros(3, n, device="cuda")
+    before = ctx.launch_count()
+    ctx.nbody_vjp(traj, stages, a_gx, a_gp)
+    mid = ctx.launch_count()
+    ctx.nbody_vjp(traj, stages, b_gx, b_gp, grad_mom_is_zero=True)
+    after = ctx.launch_count()
+    assert after - mid < mid - before                    # one backward force evaluation fewer
+    assert rel_l2(host(b_gx), host(a_gx)) < 1e-6 and rel_l2(host(b_gp), host(a_gp)) < 1e-6
+
+
+def test_binding_refuses_wrongly_shaped_arrays(fpm):
+    """a wrong shape must be an FpmError, not an out-of-bounds device access."""
+    import torch
+    ctx = fpm.FPM(32, 32)
+    n = 32 ** 3
+    pos, mom = torch.zeros(3, n, device="cuda"), torch.zeros(3, n, device="cuda")
+    with pytest.raises(fpm.FpmError):
+        ctx.nbody(pos[:, : n - 1].contiguous(), mom, [0.1, 0.2])
+    with pytest.raises(fpm.FpmError):
+        ctx.nbody(pos, mom, [0.1, 0.2], traj=torch.zeros(1, 3, n, device="cuda"))
+    with pytest.raises(fpm.FpmError):
+        ctx.paint(pos, out=torch.zeros(16, 16, 16, device="cuda"))
+    with pytest.raises(fpm.FpmError):
+        ctx.paint(torch.zeros(n, 3, device="cuda"))
+    with pytest.raises(fpm.FpmError):
+        ctx.fft_r2c(torch.zeros(32, 32, 16, device="cuda"))
+    with pytest.raises(fpm.FpmError):
+        ctx.nbody_vjp(torch.zeros(2, 3, n, device="cuda"), [0.1, 0.2, 0.3], pos, mom)
+    with pytest.raises(fpm.FpmError):
+        ctx.lpt_init(torch.zeros(16, 16, 16, device="cuda"), 0.1, 2)
+
+
 @pytest.mark.parametrize("order,np_side,ng", [(1, 32, 32), (2, 32, 32), (2, 32, 64), (2, 64, 64)])
 def test_lpt_init_vjp_matches_oracle(fpm, oracle, order, np_side, ng):
     delta = fi.linear_field(np_side, 100.0, 4)

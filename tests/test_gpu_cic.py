@@ -114,3 +114,75 @@ def test_brick_paint_with_resolution_factor_two(fpm, oracle, mode):
     got = host(ctx.paint(dev(pos), mass=dev(mass)))
     ref = oracle.paint(pos.astype(np.float64), ng, mass=mass.astype(np.float64))
     assert rel_l2(got, ref) < TOL
+
+
+def _lattice(nps, ng, sigma, seed):
+    rng = np.random.default_rng(seed)
+    q = np.stack(np.meshgrid(*[np.arange(nps) * float(ng // nps)] * 3, indexing="ij")).reshape(3, -1)
+    return np.mod(q + rng.normal(0.0, sigma, size=q.shape), ng).astype(np.float32)
+
+
+@pytest.mark.parametrize("nps,ng", [(32, 32), (64, 64), (32, 64)])
+def test_brick_paint_max_abs_error_and_window_wrap(fpm, oracle, nps, ng):
+    """Max-abs (not only L2) bound on the brick-window paint.  np = ng = 32: the 40-cell window is wider than
+    the box, so window cells alias and the flush must still add every deposit once.  Fixed-point quantum is
+    2^-19 m (2^-21 m at B = 2) per deposit and a cell of this cloud receives < 64 deposits."""
+    m0 = float((ng // nps) ** 3)
+    for sigma in (0.4, 2.5):          # inside the window / many particles on the slow path
+        pos = _lattice(nps, ng, sigma, seed=nps + ng)
+        ref = oracle.paint(pos.astype(np.float64), ng, mass_const=m0)
+        for mode in (fpm.PAINT_BRICK_FIXED, fpm.PAINT_BRICK_FLOAT, fpm.PAINT_DIRECT):
+            ctx = fpm.FPM(ng, nps, workspace=False, paint_mode=mode)
+            got = host(ctx.paint(dev(pos))).astype(np.float64)
+            assert np.max(np.abs(got - ref)) < 2e-6 * np.max(ref) + 64 * 2.0 ** -20 * m0, (sigma, mode)
+            assert rel_l2(got, ref) < TOL
+
+
+def test_fixed_point_window_cannot_overflow(fpm, oracle):
+    """All 4096 particles of a brick in ONE cell (the case the scale 2^19 / m is derived for), with the
+    constant mass, with equal negative masses and with alternating signs."""
+    nps = ng = 64
+    n = nps ** 3
+    pos = np.empty((3, n), dtype=np.float32)
+    pos[0], pos[1], pos[2] = 20.25, 21.5, 22.75
+    ctx = fpm.FPM(ng, nps, workspace=False, paint_mode=fpm.PAINT_BRICK_FIXED)
+    p64 = pos.astype(np.float64)
+    cases = [None, -np.ones(n, dtype=np.float32), np.where(np.arange(n) % 2 == 0, 1.0, -1.0).astype(np.float32),
+             np.full(n, 32768.0, dtype=np.float32)]
+    for mass in cases:
+        got = host(ctx.paint(dev(pos), None if mass is None else dev(mass))).astype(np.float64)
+        ref = oracle.paint(p64, ng, mass=None if mass is None else mass.astype(np.float64), mass_const=1.0)
+        scale = max(np.max(np.abs(ref)), float(n) * (1.0 if mass is None else float(np.max(np.abs(mass)))) / 64)
+        assert np.max(np.abs(got - ref)) < 2e-6 * scale
+        assert np.count_nonzero(got) <= 8
+
+
+def test_paint_with_badly_conditioned_and_non_finite_masses(fpm, oracle):
+    """a brick with one huge outlier must not coarsen its ordinary deposits, and NaN/Inf masses
+    must propagate (AUTO keeps the fixed-point window only for well-conditioned bricks)."""
+    nps = ng = 64
+    n = nps ** 3
+    pos = _lattice(nps, ng, 0.7, seed=5)
+    rng = np.random.default_rng(9)
+    mass = np.exp(rng.normal(0.0, 1.0, n)).astype(np.float32)            # log-normal, heavy-ish tail
+    mass[12345] = 1.0e6                                                   # one outlier
+    mass[54321] = -3.0e5
+    ctx = fpm.FPM(ng, nps, workspace=False)                               # PAINT_AUTO
+    got = host(ctx.paint(dev(pos), dev(mass))).astype(np.float64)
+    ref = oracle.paint(pos.astype(np.float64), ng, mass=mass.astype(np.float64))
+    # well away from the outliers the error must stay at the level of ordinary masses (mean ~ 1.6):
+    # 2^-18 mean|m| per deposit, < 64 deposits per cell; near them fp32 rounding of the outlier itself
+    err = np.abs(got - ref)
+    assert np.max(err - 2e-7 * np.abs(ref)) < 64 * 2.0 ** -18 * 2.0
+    assert rel_l2(got, ref) < 1e-6
+    bad = mass.copy()
+    bad[777] = np.nan
+    bad[100000] = np.inf
+    got = host(ctx.paint(dev(pos), dev(bad)))
+    i777 = np.floor(pos[:, 777]).astype(int)
+    i1e5 = np.floor(pos[:, 100000]).astype(int)
+    assert np.isnan(got[tuple(i777)]) and not np.isfinite(got[tuple(i1e5)])
+    finite_ref = oracle.paint(pos.astype(np.float64), ng, mass=np.where(np.isfinite(bad), mass, 0.0).astype(np.float64))
+    ok = np.isfinite(got)
+    assert ok.sum() >= got.size - 16
+    assert np.max(np.abs(got[ok] - finite_ref[ok])) < 1e-3

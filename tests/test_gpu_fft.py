@@ -38,6 +38,20 @@ def test_r2c_and_c2r_match_oracle(fpm, oracle, ng):
     assert rel_l2(rt, rho) < TOL
 
 
+@pytest.mark.parametrize("ng", [16, 64])
+def test_c2r_of_a_non_hermitian_spectrum_follows_the_stated_contract(fpm, oracle, ng):
+    """include/fpm.h, fpm_fft_c2r: on a spectrum whose kz = 0 / Nyquist planes are not Hermitian the result is
+    the real part of the inverse of the conjugate-completed spectrum -- what the oracle computes (pinned
+    against numpy.fft.ifftn in tests/test_oracle_fft.py)."""
+    rng = np.random.default_rng(ng + 1)
+    spec = (rng.standard_normal((ng, ng, ng // 2 + 1)) + 1j * rng.standard_normal((ng, ng, ng // 2 + 1))).astype(np.complex64)
+    ctx = fpm.FPM(ng, workspace=False)
+    got = host(ctx.fft_c2r(dev(spec)))
+    ref = oracle.fft_c2r(spec.astype(np.complex128))
+    assert rel_l2(got, ref) < TOL
+    assert np.max(np.abs(got - ref)) < 1e-5 * np.max(np.abs(ref))
+
+
 def test_delta_and_plane_wave_closed_forms(fpm):
     ng = 64
     ctx = fpm.FPM(ng, workspace=False)
@@ -53,19 +67,21 @@ def test_delta_and_plane_wave_closed_forms(fpm):
     assert np.max(np.abs(got - expect)) < 2e-6 * ng ** 3
 
 
-@pytest.mark.parametrize("ng", [512])
+@pytest.mark.parametrize("ng", [512, 1024])
 def test_full_size_sampled_outputs_and_roundtrip(fpm, ng):
-    """At the bench size the oracle computes sampled output bins one by one (direct DFT sums)."""
+    """At the bench sizes (C4: 512, C5: 1024 -- Plan<1024>, the 128 KB column tiles and the M = 512 z pass)
+    the oracle computes sampled output bins one by one (direct DFT sums)."""
     import torch
     rng = np.random.default_rng(1)
-    rho = rng.standard_normal((ng, ng, ng)).astype(np.float32)
+    rho = rng.standard_normal((ng, ng, ng), dtype=np.float32)
     ctx = fpm.FPM(ng, workspace=False)
     d_rho = dev(rho)
     spec = ctx.fft_r2c(d_rho)
     x = np.arange(ng)
     r64 = rho.astype(np.float64)
     scale = np.sqrt(ng ** 3)
-    for (a, b, c) in [(0, 0, 0), (1, 2, 3), (511, 256, 256), (257, 13, 0), (100, 300, 77), (256, 256, 256)]:
+    h = ng // 2
+    for (a, b, c) in [(0, 0, 0), (1, 2, 3), (ng - 1, h, h), (h + 1, 13, 0), (100, 300, 77), (h, h, h)]:
         ea = np.exp(-2j * np.pi * a * x / ng)
         eb = np.exp(-2j * np.pi * b * x / ng)
         ec = np.exp(-2j * np.pi * c * x / ng)

@@ -47,6 +47,31 @@ def test_growth_and_factors_match_oracle(fpm, oracle):
     assert cq.kick_factor(0.1, 0.2, 0.3) == pytest.approx(oracle.kick_factor(OM, 0.1, 0.2, 0.3, 1), rel=1e-9)
 
 
+def test_step_factors_are_the_merged_leapfrog_factors(fpm, oracle):
+    """fpm_step_factors (R6): half step at sqrt(a_j a_j+1); the second half kick of step j-1 and the first of
+    step j share one force evaluation.  Rebuilt here from the oracle's kick/drift factors."""
+    stages = fi.CONFIGS["C2"].stages()
+    n = len(stages) - 1
+    for factor_mode in (0, 1):
+        ctx = fpm.FPM(16, factor_mode=factor_mode, workspace=False)
+        got = ctx.step_factors(stages)
+        assert len(got) == n + 1
+        pending = 0.0
+        for j in range(n + 1):
+            kf, dr = pending, 0.0
+            if j < n:
+                ai, af = stages[j], stages[j + 1]
+                ah = (ai * af) ** 0.5
+                kf += oracle.kick_factor(OM, ai, ai, ah, factor_mode)
+                dr = oracle.drift_factor(OM, ai, ah, af, factor_mode)
+                pending = oracle.kick_factor(OM, ah, af, af, factor_mode)
+            assert got[j][0] == pytest.approx(kf, rel=1e-7) and got[j][1] == pytest.approx(dr, rel=1e-7, abs=0.0)
+    assert got[n][1] == 0.0
+    assert ctx.step_factors([0.5]) == [(0.0, 0.0)]
+    with pytest.raises(fpm.FpmError):
+        ctx.step_factors([0.1, -0.2])
+
+
 @pytest.mark.parametrize("force_path", [0, 1])
 @pytest.mark.parametrize("ng,nps,mode", [(32, 32, 0), (64, 32, 0), (64, 64, 1), (64, 64, 2), (128, 128, 0)])
 def test_force_evaluation_matches_oracle(fpm, oracle, ng, nps, mode, force_path):

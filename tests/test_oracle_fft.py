@@ -76,3 +76,21 @@ def test_parseval_with_half_space_weights(oracle):
     w = np.full(ng // 2 + 1, 2.0)
     w[0] = w[-1] = 1.0
     assert np.sum(w * np.abs(spec) ** 2) / ng ** 3 == pytest.approx(np.sum(rho ** 2), rel=1e-12)
+
+
+def test_c2r_of_a_spectrum_that_is_not_hermitian_on_the_kz_0_and_nyquist_planes(oracle):
+    """The contract include/fpm.h states for fpm_fft_c2r on inputs that are not the spectrum of a real
+    field: the result is the real part of the inverse transform of the spectrum completed by
+    a(-k) = conj(a(k)) for 0 < kz < ng/2, with the planes kz = 0 and kz = ng/2 taken as stored.
+    Pinned against numpy.fft.ifftn of the explicitly completed full spectrum."""
+    ng = 8
+    rng = np.random.default_rng(11)
+    half = rng.standard_normal((ng, ng, ng // 2 + 1)) + 1j * rng.standard_normal((ng, ng, ng // 2 + 1))
+    full = np.zeros((ng, ng, ng), dtype=np.complex128)
+    full[:, :, : ng // 2 + 1] = half
+    idx = (-np.arange(ng)) % ng
+    for z in range(ng // 2 + 1, ng):
+        full[:, :, z] = np.conj(half[idx][:, idx][:, :, ng - z])
+    ref = np.fft.ifftn(full).real
+    assert np.max(np.abs(oracle.fft_c2r(half) - ref)) < 1e-13
+    assert np.max(np.abs(oracle.fft_c2r(half, force_naive=True) - ref)) < 1e-13

@@ -79,6 +79,29 @@ def _plane_wave_growth(oracle, n, mode_number, n_steps=5):
     return np.array(out)
 
 
+@pytest.mark.parametrize("order,n,ng", [(1, 8, 8), (2, 8, 8), (1, 8, 16), (2, 8, 16)])
+def test_lpt_momenta_are_the_time_derivative_of_the_lpt_positions(oracle, order, n, ng):
+    """Independent pin of the momentum coefficients a^2 E f1 D1 and a^2 E f2 D2 (Alg. 4, PAPER.md:363-383;
+    R0: p = a^2 dx/dt / H0 = a^3 E dx/da): a 4th-order central difference in a0 of the oracle's own LPT
+    POSITIONS must reproduce its momenta.  E(a) is typed out from its definition (R0), not taken from
+    oracle.growth, so a wrong f1, f2, D2 normalisation or a missing factor of a fails here (the D(a) pin
+    of the plane-wave test cannot see f(a): f1(0.1) = 0.9988)."""
+    a0, h = 0.1, 2e-3
+    delta = 0.05 * fi.linear_field(n, 50.0, seed=3).astype(np.float64)
+
+    def x_of(a):
+        return oracle.lpt_init(delta, ng, OM, a, order)[0]
+
+    def wrapped_diff(u, v):
+        d = u - v
+        return d - ng * np.round(d / ng)
+
+    dxda = (8.0 * wrapped_diff(x_of(a0 + h), x_of(a0 - h)) - wrapped_diff(x_of(a0 + 2 * h), x_of(a0 - 2 * h))) / (12.0 * h)
+    e_of_a = math.sqrt(OM / a0 ** 3 + 1.0 - OM)
+    _, mom = oracle.lpt_init(delta, ng, OM, a0, order)
+    assert np.max(np.abs(a0 ** 3 * e_of_a * dxda - mom)) < 1e-6 * np.max(np.abs(mom))
+
+
 def test_small_plane_wave_follows_linear_growth(oracle):
     """ICs from the Zel'dovich approximation at a = 0.1, 5 steps to a = 1: the displacement
     amplitude tracks D1(a) up to the paint x readout window and the finite-difference kernels,

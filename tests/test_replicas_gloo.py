@@ -60,3 +60,29 @@ def test_single_process_needs_no_process_group():
     assert rep.env_world() == (0, 0, 1)
     assert rep.max_over_ranks(3.5) == 3.5
     assert rep.whole_job_rate(4, 2.0, 1) == 2000.0
+
+
+def test_bench_style_self_launch_of_two_replicas(tmp_path):
+    """`bench.py --gpus N` without torchrun must start N ranks itself: needs_spawn + launch_command
+    run a two-rank gloo job that reports WORLD_SIZE, the per-rank seeds and the max-over-ranks."""
+    import subprocess
+    rep = _load_replicas()
+    for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"):
+        os.environ.pop(k, None)
+    assert rep.needs_spawn(2) and not rep.needs_spawn(1)
+    script = tmp_path / "ranks.py"
+    script.write_text(
+        "import importlib.util, os, sys\n"
+        f"spec = importlib.util.spec_from_file_location('r', {os.path.join(ROOT, 'paper_2010_11847_b200', 'replicas.py')!r})\n"
+        "rep = importlib.util.module_from_spec(spec); spec.loader.exec_module(rep)\n"
+        "assert not rep.needs_spawn(int(sys.argv[1]))\n"
+        "rank, local, world = rep.init('gloo')\n"
+        "ms = rep.max_over_ranks(1.0 + rank)\n"
+        "print('RANK', rank, world, rep.replica_seed(1, rank), ms, flush=True)\n"
+        "rep.finalize()\n")
+    cmd = rep.launch_command(2, str(script), ["2"])
+    assert "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = sorted(l for l in out.stdout.splitlines() if l.startswith("RANK"))
+    assert lines == ["RANK 0 2 1 2.0", "RANK 1 2 2 2.0"]
