@@ -295,6 +295,51 @@ def side_measurements(args, ctx, cfg, pos, mom, factors, device):
                               "loss_after_11_iterations": state["loss"],
                               "paper_context": "1.1 s/iteration on one V100, 4.6 s on 128 Haswell cores (PAPER.md:502)"}
     rctx.close()
+    del truth, p0, m0, data, ipow, s, am, av
+    torch.cuda.empty_cache()
+    # (iv) SURVEY.md 8(f) N2: batched small simulations.  B independent C1 / C2 runs advance
+    # in the same kernel launches and the whole run replays as one CUDA graph; compared with ONE simulation
+    # run kernel by kernel (round 1's path) and with one simulation replayed as a graph.
+    peak, _ = measured_peaks()
+    out["batched_small_sims"] = {}
+    for name, batch in (("C1", 64), ("C2", 16)):
+        c = fi.CONFIGS[name]
+        n_ev = c.n_steps + 1
+
+        def run_rate(b, graph_mode, reps):
+            bctx = fpm.FPM(c.ng, c.np_side, omega_m=fi.COSMO["omega_m"], box=c.box, device=device,
+                           force_path=fpm.FORCE_FUSED, batch=b)
+            bctx.set_graph_mode(graph_mode)
+            fields = np.stack([fi.linear_field(c.np_side, c.box, c.seed + i) for i in range(b)])
+            d = torch.from_numpy(fields if b > 1 else fields[0]).to(device)
+            q0, r0 = bctx.lpt_init(d, c.a0, c.lpt_order)
+            q, r = q0.clone(), r0.clone()
+            bctx.nbody(q, r, c.stages())                      # warm-up (captures the graph when one is used)
+            torch.cuda.synchronize()
+            total = 0.0
+            for _ in range(reps):
+                q.copy_(q0)
+                r.copy_(r0)
+                a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                bctx.nbody(q, r, c.stages())
+                z.record()
+                torch.cuda.synchronize()
+                total += a.elapsed_time(z)
+            bctx.close()
+            return b * n_ev * reps * 1e3 / total, total / reps
+
+        one_eager, _ = run_rate(1, fpm.GRAPH_OFF, 20)
+        one_graph, _ = run_rate(1, fpm.GRAPH_ALWAYS, 20)
+        many, ms_run = run_rate(batch, fpm.GRAPH_AUTO, 10)
+        step_bytes = batch * step_bytes_fused_path(c.n_particles, c.ng)
+        out["batched_small_sims"][f"{batch}x{name}"] = {
+            "call": "fpm_nbody on a batch context (one CUDA graph launch per run)",
+            "pm_steps_per_s_aggregate": many, "particle_updates_per_s": many * c.n_particles,
+            "ms_per_run": ms_run, "force_evaluations_per_run": n_ev,
+            "step_roofline_frac": step_bytes * n_ev / (ms_run * 1e-3) / 1e9 / peak,
+            "one_sim_kernel_by_kernel_steps_per_s": one_eager, "one_sim_graph_steps_per_s": one_graph,
+            "speedup_vs_one_sim_kernel_by_kernel": many / one_eager}
     return out
 
 

@@ -91,7 +91,18 @@ typedef struct {
   int32_t factor_mode; /* FPM_FACTORS_* */
   int32_t force_path;  /* FPM_FORCE_* */
   int32_t paint_mode;  /* FPM_PAINT_* */
+  int32_t batch;       /* independent simulations advanced together (0 or 1: one); see "Batches" below */
 } fpm_config;
+
+/* Batches ("splitting along the batch dimension is almost always the most
+ * efficient"): with batch = B > 1 a context advances B independent simulations of the same
+ * (ng, np, cosmology) in the SAME kernel launches -- every kernel's grid is extended over the batch, so small
+ * configurations stop being bound by launch latency.  Particle arrays are then [B][3][n], the linear field of
+ * fpm_lpt_init [B][np^3], meshes [B][ng^3]; `n` stays the particle count of ONE simulation.  Simulation b's
+ * results equal those of a batch-1 run of the same inputs.  Calls that take a batch: fpm_lpt_init, fpm_paint,
+ * fpm_pm_step, fpm_nbody (traj: [n_steps+1][B][3][n]); the batch needs FPM_FORCE_FUSED and a full np^3
+ * lattice particle set (np a multiple of 32); every other call returns FPM_ENOTIMPL on a context with
+ * batch > 1. */
 
 typedef struct fpm_ctx fpm_ctx;
 
@@ -114,6 +125,13 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes);
 
 /* Changes cfg.paint_mode after creation.  FPM_EINVAL on an unknown mode. */
 int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode);
+
+/* How fpm_nbody enqueues its n_steps + 1 PM steps.  FPM_GRAPH_AUTO [default]: when one PM step is small enough
+ * to be bound by launch latency (batch * ng^3 <= 2^24 cells), the whole run is captured once into a CUDA graph
+ * (cached per argument set on the context) and replayed with one launch; larger runs enqueue kernel by kernel.
+ * Results are identical either way. */
+enum { FPM_GRAPH_OFF = 0, FPM_GRAPH_AUTO = 1, FPM_GRAPH_ALWAYS = 2 };
+int fpm_set_graph_mode(fpm_ctx* ctx, int graph_mode);
 
 /* ---- background cosmology (host, float64; paper defers to Feng et al. 2016) -- */
 /* out: HOST double[7] = {D1, f1, D2, f2, E, Gf = a^3 E dD1/da, gf = dGf/da}, D1(1) = 1. */

@@ -185,6 +185,53 @@ def nbody(pos, mom, ng, np_side, omega_m, stages, mode=KERNEL_PAPER, factor_mode
     return (pos, mom, traj) if return_traj else (pos, mom)
 
 
+def reduce(mesh, levels=2):
+    """Alg. 2 REDUCE (reading R14): f stride-2 convolutions with the order-6 B-spline mask."""
+    m = _f64(mesh)
+    n = m.shape[0]
+    out = np.zeros((n >> levels,) * 3)
+    _load().orc_reduce(_p(m), ctypes.c_int(n), ctypes.c_int(levels), _p(out))
+    return out
+
+
+def expand(mesh, levels=2):
+    """Alg. 2 EXPAND: f transposed stride-2 convolutions with 8 x the same mask."""
+    m = _f64(mesh)
+    n = m.shape[0]
+    out = np.zeros((n << levels,) * 3)
+    _load().orc_expand(_p(m), ctypes.c_int(n), ctypes.c_int(levels), _p(out))
+    return out
+
+
+def force_grids_pyramid(rho, levels=2, mode=KERNEL_PAPER, scale=1.0):
+    """Alg. 3 Force(H, f): the three force meshes of the two-level pyramid scheme."""
+    rho = _f64(rho)
+    ng = rho.shape[0]
+    outs = [np.zeros((ng, ng, ng)) for _ in range(3)]
+    _load().orc_force_grids_pyramid(_p(rho), ctypes.c_int(ng), ctypes.c_int(mode), ctypes.c_double(scale),
+                                    ctypes.c_int(levels), *[_p(o) for o in outs])
+    return outs
+
+
+def force_pyramid(pos, ng, levels=2, mode=KERNEL_PAPER, scale=1.0, mass=1.0):
+    pos = _f64(pos)
+    n = pos.shape[1]
+    f = np.zeros((3, n))
+    _load().orc_force_pyramid(_p(pos), ctypes.c_int64(n), ctypes.c_int(ng), ctypes.c_int(mode),
+                              ctypes.c_double(scale), ctypes.c_double(mass), ctypes.c_int(levels), _p(f))
+    return f
+
+
+def nbody_batch(pos, mom, ng, np_side, omega_m, stages, mode=KERNEL_PAPER, factor_mode=FACTORS_FASTPM):
+    """SURVEY.md 8(f) N2 (the batch dimension): a batch of B simulations IS B independent
+    runs -- the definition written out as the loop it is.  pos, mom: [B][3][n]; returns the final [B][3][n]."""
+    pos, mom = _f64(pos), _f64(mom)
+    out_p, out_m = np.empty_like(pos), np.empty_like(mom)
+    for b in range(pos.shape[0]):
+        out_p[b], out_m[b] = nbody(pos[b], mom[b], ng, np_side, omega_m, stages, mode, factor_mode)
+    return out_p, out_m
+
+
 def power(mesh_a, box, mesh_b=None):
     """(k_mean, P(k), N_modes) in bins centred on integer multiples of k_f (R13)."""
     a = _f64(mesh_a)

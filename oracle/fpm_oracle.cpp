@@ -346,6 +346,104 @@ void force_grids_impl(const double* rho, int ng, int mode, double scale, double*
   for (int d = 0; d < 3; ++d) c2r_impl(fk[d], ng, F[d], false);
 }
 
+// ------------------------------------------------------------------------------------------
+// N3  Multi-grid pyramid (Eq. 6-9; Alg. 2-3).  DESIGN.md reading R14:
+//   * BSpline(6): the paper names "a 3-D bspline kernel of order 6" and nothing else.  Taken as the two-scale
+//     (refinement) mask of the order-6 cardinal B-spline, h = [1, 6, 15, 20, 15, 6, 1] / 64 per axis, offsets
+//     -3..3, K = h (x) h (x) h, sum 1: the low-pass for which upsampling by EXPAND is exact B-spline
+//     subdivision, and the one whose transposed filter needs the paper's factor 8 = 2^3 to interpolate
+//     (each polyphase of 2 h sums to 1).
+//   * Conv3D(D, K, S = 2), periodic:        out[X] = sum_j K[j] in[(2 X + j) mod n]            (n -> n/2)
+//   * TransposedConv3D(H, 8 K, S = 2):      out[x] = sum_X 8 K[x - 2 X] in[X]  (periodic)     (n/2 -> n)
+//   * REDUCE / EXPAND apply them f times (Alg. 2: "consecutively f times").
+//   * Force (Alg. 3): F = EXPAND(2^f ForceGrids(REDUCE(H))) + F_S - EXPAND(REDUCE(F_S)), F_S = ForceGrids(H).
+//     The factor 2^f is units: ForceGrids on the coarse mesh gives the force per COARSE cell spacing
+//     (laplace^-1 ~ spacing^2, grad ~ 1/spacing), and one coarse spacing is 2^f fine cells; Alg. 3 is silent.
+// Plain loops over the definition; nothing separable, nothing cached.
+// ------------------------------------------------------------------------------------------
+const double kBspline6[7] = {1.0 / 64, 6.0 / 64, 15.0 / 64, 20.0 / 64, 15.0 / 64, 6.0 / 64, 1.0 / 64};
+
+// one level: in [n^3] -> out [(n/2)^3]
+void conv3d_stride2(const double* in, int n, double* out) {
+  const int64_t m = n / 2, g = n;
+#pragma omp parallel for schedule(static)
+  for (int64_t X = 0; X < m; ++X)
+    for (int64_t Y = 0; Y < m; ++Y)
+      for (int64_t Z = 0; Z < m; ++Z) {
+        double s = 0.0;
+        for (int a = -3; a <= 3; ++a)
+          for (int b = -3; b <= 3; ++b)
+            for (int c = -3; c <= 3; ++c) {
+              const int64_t x = wrap_index(2 * X + a, g), y = wrap_index(2 * Y + b, g), z = wrap_index(2 * Z + c, g);
+              s += kBspline6[a + 3] * kBspline6[b + 3] * kBspline6[c + 3] * in[(x * g + y) * g + z];
+            }
+        out[(X * m + Y) * m + Z] = s;
+      }
+}
+
+// one level: in [m^3] -> out [(2m)^3], kernel 8 K
+void transposed_conv3d_stride2(const double* in, int m_, double* out) {
+  const int64_t m = m_, g = 2 * m;
+  std::memset(out, 0, sizeof(double) * g * g * g);
+  // scatter form of the definition: coarse cell X contributes 8 K[j] in[X] to fine cell 2 X + j
+  for (int64_t X = 0; X < m; ++X)
+    for (int64_t Y = 0; Y < m; ++Y)
+      for (int64_t Z = 0; Z < m; ++Z) {
+        const double v = 8.0 * in[(X * m + Y) * m + Z];
+        for (int a = -3; a <= 3; ++a)
+          for (int b = -3; b <= 3; ++b)
+            for (int c = -3; c <= 3; ++c) {
+              const int64_t x = wrap_index(2 * X + a, g), y = wrap_index(2 * Y + b, g), z = wrap_index(2 * Z + c, g);
+              out[(x * g + y) * g + z] += kBspline6[a + 3] * kBspline6[b + 3] * kBspline6[c + 3] * v;
+            }
+      }
+}
+
+// Alg. 2 REDUCE(H, f): in [n^3] -> out [(n / 2^f)^3]
+void reduce_impl(const double* in, int n, int f, double* out) {
+  std::vector<double> cur(in, in + (int64_t)n * n * n), nxt;
+  for (int i = 0; i < f; ++i) {
+    const int64_t m = n / 2;
+    nxt.assign(m * m * m, 0.0);
+    conv3d_stride2(cur.data(), n, nxt.data());
+    cur.swap(nxt);
+    n = (int)m;
+  }
+  std::memcpy(out, cur.data(), sizeof(double) * cur.size());
+}
+
+// Alg. 2 EXPAND(D, f): in [m^3] -> out [(m 2^f)^3]
+void expand_impl(const double* in, int m, int f, double* out) {
+  std::vector<double> cur(in, in + (int64_t)m * m * m), nxt;
+  for (int i = 0; i < f; ++i) {
+    const int64_t g = 2 * (int64_t)m;
+    nxt.assign(g * g * g, 0.0);
+    transposed_conv3d_stride2(cur.data(), m, nxt.data());
+    cur.swap(nxt);
+    m = (int)g;
+  }
+  std::memcpy(out, cur.data(), sizeof(double) * cur.size());
+}
+
+// Alg. 3 Force(H, f): the three force meshes of the two-level pyramid scheme, in the paper's order
+void force_grids_pyramid_impl(const double* rho, int ng, int mode, double scale, int f, double* F[3]) {
+  const int nc = ng >> f;
+  const int64_t g3 = (int64_t)ng * ng * ng, c3 = (int64_t)nc * nc * nc;
+  std::vector<double> D(c3);
+  reduce_impl(rho, ng, f, D.data());                                   // D <= REDUCE(H)
+  std::vector<double> FL0(c3), FL1(c3), FL2(c3);
+  double* FL[3] = {FL0.data(), FL1.data(), FL2.data()};
+  force_grids_impl(D.data(), nc, mode, scale * (double)(1 << f), FL);  // F_L <= ForceGrids(D), in fine-cell units
+  force_grids_impl(rho, ng, mode, scale, F);                           // F_S <= ForceGrids(H)
+  std::vector<double> up(g3), low(c3), lowup(g3);
+  for (int d = 0; d < 3; ++d) {
+    expand_impl(FL[d], nc, f, up.data());                              // F_iL <= EXPAND(F_iL)
+    reduce_impl(F[d], ng, f, low.data());                              // F_il <= REDUCE(F_iS)
+    expand_impl(low.data(), nc, f, lowup.data());                      // F_il <= EXPAND(F_il)
+    for (int64_t i = 0; i < g3; ++i) F[d][i] = up[i] + (F[d][i] - lowup[i]);   // F_i <= F_iL + (F_iS - F_il)
+  }
+}
+
 // paint -> ForceGrids -> readout x3 : one force evaluation at the particles.
 void force_impl(const double* pos, int64_t n, int ng, int mode, double scale, double mass,
                 double* force, double* rho_out) {
@@ -805,6 +903,24 @@ void orc_force_grids(const double* rho, int ng, int mode, double scale, double* 
 void orc_force(const double* pos, int64_t n, int ng, int mode, double scale, double mass,
                double* force, double* rho_out) {
   force_impl(pos, n, ng, mode, scale, mass, force, rho_out);
+}
+
+void orc_reduce(const double* in, int n, int f, double* out) { reduce_impl(in, n, f, out); }
+void orc_expand(const double* in, int m, int f, double* out) { expand_impl(in, m, f, out); }
+void orc_force_grids_pyramid(const double* rho, int ng, int mode, double scale, int f, double* Fx, double* Fy,
+                             double* Fz) {
+  double* F[3] = {Fx, Fy, Fz};
+  force_grids_pyramid_impl(rho, ng, mode, scale, f, F);
+}
+// one pyramid force evaluation at the particles: paint -> Alg. 3 Force -> readout x3
+void orc_force_pyramid(const double* pos, int64_t n, int ng, int mode, double scale, double mass, int f,
+                       double* force) {
+  const int64_t g3 = (int64_t)ng * ng * ng;
+  std::vector<double> rho(g3), F0(g3), F1(g3), F2(g3);
+  paint_impl(pos, nullptr, mass, n, ng, rho.data());
+  double* F[3] = {F0.data(), F1.data(), F2.data()};
+  force_grids_pyramid_impl(rho.data(), ng, mode, scale, f, F);
+  for (int d = 0; d < 3; ++d) readout_impl(F[d], pos, n, ng, force + d * n);
 }
 
 void orc_kick(double* mom, const double* force, int64_t n, double factor) {

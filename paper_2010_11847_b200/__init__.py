@@ -18,6 +18,7 @@ KERNEL_PAPER, KERNEL_NAIVE, KERNEL_MIXED = 0, 1, 2
 FACTORS_FASTPM, FACTORS_QUINN = 0, 1
 FORCE_UNFUSED, FORCE_FUSED = 0, 1
 PAINT_AUTO, PAINT_DIRECT, PAINT_BRICK_FLOAT, PAINT_BRICK_FIXED = 0, 1, 2, 3
+GRAPH_OFF, GRAPH_AUTO, GRAPH_ALWAYS = 0, 1, 2
 VJP_GRAD_MOM_ZERO = 1
 OK, EINVAL, ENOMEM, ECUDA, ENOTIMPL = 0, -1, -2, -3, -4
 
@@ -30,7 +31,7 @@ class _Config(ctypes.Structure):
     _fields_ = [("ng", ctypes.c_int32), ("np", ctypes.c_int32), ("omega_m", ctypes.c_double),
                 ("box", ctypes.c_double), ("kernel_mode", ctypes.c_int32),
                 ("factor_mode", ctypes.c_int32), ("force_path", ctypes.c_int32),
-                ("paint_mode", ctypes.c_int32)]
+                ("paint_mode", ctypes.c_int32), ("batch", ctypes.c_int32)]
 
 
 def _load():
@@ -49,6 +50,7 @@ def _load():
         "fpm_workspace_bytes": (ctypes.c_size_t, [ctypes.POINTER(_Config)]),
         "fpm_set_workspace": (i32, [vp, vp, ctypes.c_size_t]),
         "fpm_set_paint_mode": (i32, [vp, i32]),
+        "fpm_set_graph_mode": (i32, [vp, i32]),
         "fpm_growth": (i32, [vp, dbl, ctypes.POINTER(dbl)]),
         "fpm_drift_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
         "fpm_kick_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
@@ -112,11 +114,16 @@ def _dev(t, dtype=torch.float32, numel=None, what="tensor"):
     return ctypes.c_void_p(t.data_ptr())
 
 
-def _particles(t, what="pos"):
-    """[3][n] particle array -> n."""
-    if not (isinstance(t, torch.Tensor) and t.dim() == 2 and t.shape[0] == 3):
-        raise FpmError(f"{what}: expected a [3][n] tensor, got shape {tuple(getattr(t, 'shape', ()))}")
-    return int(t.shape[1])
+def _particles(t, what="pos", batch=1):
+    """[3][n] particle array ([batch][3][n] on a batched context) -> n, the particle count of one simulation."""
+    shape = tuple(getattr(t, "shape", ()))
+    if batch > 1:
+        if not (isinstance(t, torch.Tensor) and len(shape) == 3 and shape[0] == batch and shape[1] == 3):
+            raise FpmError(f"{what}: expected a [{batch}][3][n] tensor on a batched context, got shape {shape}")
+        return int(shape[2])
+    if not (isinstance(t, torch.Tensor) and len(shape) == 2 and shape[0] == 3):
+        raise FpmError(f"{what}: expected a [3][n] tensor, got shape {shape}")
+    return int(shape[1])
 
 
 class FPM:
@@ -124,7 +131,7 @@ class FPM:
 
     def __init__(self, ng, np_side=None, omega_m=0.3075, box=0.0, kernel_mode=KERNEL_PAPER,
                  factor_mode=FACTORS_FASTPM, force_path=FORCE_UNFUSED, device="cuda:0",
-                 stream=None, workspace=True, paint_mode=PAINT_AUTO):
+                 stream=None, workspace=True, paint_mode=PAINT_AUTO, batch=1):
         if not torch.cuda.is_available():
             raise FpmError("CUDA device required: libfpm has no CPU fallback")
         self.device = torch.device(device)
@@ -132,8 +139,9 @@ class FPM:
         self.n_particles = self.np_side ** 3
         self.nzh = self.ng // 2 + 1
         self.omega_m = float(omega_m)
+        self.batch = int(batch)
         self._cfg = _Config(self.ng, self.np_side, self.omega_m, float(box), kernel_mode,
-                            factor_mode, force_path, paint_mode)
+                            factor_mode, force_path, paint_mode, self.batch)
         with torch.cuda.device(self.device):
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = ctypes.c_void_p()
@@ -170,6 +178,9 @@ class FPM:
     def set_paint_mode(self, mode):
         self._check(_lib.fpm_set_paint_mode(self._h, int(mode)))
 
+    def set_graph_mode(self, mode):
+        self._check(_lib.fpm_set_graph_mode(self._h, int(mode)))
+
     # ---- cosmology ----------------------------------------------------------------------
     def growth(self, a):
         out = (ctypes.c_double * 7)()
@@ -198,10 +209,12 @@ class FPM:
         return self.ng * self.ng * self.nzh
 
     def paint(self, pos, mass=None, out=None):
-        n = _particles(pos)
-        mesh = out if out is not None else self._empty(self.ng, self.ng, self.ng)
-        self._check(_lib.fpm_paint(self._h, _dev(pos), _dev(mass, numel=n, what="mass"), n,
-                                   _dev(mesh, numel=self._n_g, what="mesh")))
+        b = self.batch
+        n = _particles(pos, batch=b)
+        shape = (self.ng, self.ng, self.ng) if b <= 1 else (b, self.ng, self.ng, self.ng)
+        mesh = out if out is not None else self._empty(*shape)
+        self._check(_lib.fpm_paint(self._h, _dev(pos), _dev(mass, numel=n * max(b, 1), what="mass"), n,
+                                   _dev(mesh, numel=self._n_g * max(b, 1), what="mesh")))
         return mesh
 
     def fft_r2c(self, real, out=None):
@@ -256,8 +269,10 @@ class FPM:
         return pos
 
     def lpt_init(self, delta_lin, a0, order):
-        pos, mom = self._empty(3, self.n_particles), self._empty(3, self.n_particles)
-        self._check(_lib.fpm_lpt_init(self._h, _dev(delta_lin, numel=self.n_particles, what="delta_lin"), a0,
+        b = max(self.batch, 1)
+        shape = (3, self.n_particles) if b == 1 else (b, 3, self.n_particles)
+        pos, mom = self._empty(*shape), self._empty(*shape)
+        self._check(_lib.fpm_lpt_init(self._h, _dev(delta_lin, numel=b * self.n_particles, what="delta_lin"), a0,
                                       order, _dev(pos), _dev(mom)))
         return pos, mom
 
@@ -268,15 +283,15 @@ class FPM:
 
     def nbody(self, pos, mom, stages, traj=None):
         st, n_steps = self._stages(stages)
-        n3 = 3 * self.n_particles
+        n3 = 3 * self.n_particles * max(self.batch, 1)
         self._check(_lib.fpm_nbody(self._h, _dev(pos, numel=n3, what="pos"), _dev(mom, numel=n3, what="mom"), st,
                                    n_steps, _dev(traj, numel=(n_steps + 1) * n3, what="traj")))
         return pos, mom
 
     def pm_step(self, pos, mom, kick_fac, drift_fac):
         """One PM step: force at pos, mom += f * kick_fac, pos = wrap(pos + mom * drift_fac)."""
-        n = _particles(pos)
-        self._check(_lib.fpm_pm_step(self._h, _dev(pos), _dev(mom, numel=3 * n, what="mom"), n, kick_fac,
+        n = _particles(pos, batch=self.batch)
+        self._check(_lib.fpm_pm_step(self._h, _dev(pos), _dev(mom, numel=pos.numel(), what="mom"), n, kick_fac,
                                      drift_fac))
         return pos, mom
 

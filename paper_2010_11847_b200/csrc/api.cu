@@ -15,7 +15,9 @@ namespace {
 
 inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
 inline size_t real_bytes(int n) { return align256(sizeof(float) * (size_t)n * n * n); }
-inline size_t cplx_bytes(int n) { return align256(sizeof(float2) * (size_t)n * n * (n / 2 + 1)); }
+// half-complex scratch meshes are sized for the padded internal row pitch (n/2 + 1 rounded up to 16 elements;
+// fft.cuh padded_pitch), which the dense cuFFT-layout uses of the same buffers fit inside
+inline size_t cplx_bytes(int n) { return align256(sizeof(float2) * (size_t)n * n * (size_t)((n / 2 + 1 + 15) & ~15)); }
 
 bool config_ok(const fpm_config* c) {
   if (!c) return false;
@@ -26,7 +28,20 @@ bool config_ok(const fpm_config* c) {
   if (c->factor_mode < FPM_FACTORS_FASTPM || c->factor_mode > FPM_FACTORS_QUINN) return false;
   if (c->force_path < FPM_FORCE_UNFUSED || c->force_path > FPM_FORCE_FUSED) return false;
   if (c->paint_mode < FPM_PAINT_AUTO || c->paint_mode > FPM_PAINT_BRICK_FIXED) return false;
+  if (c->batch < 0 || (int64_t)c->batch * c->ng > 65535) return false;
+  // a batch runs the fused path over Lagrangian bricks only (fpm.h "Batches")
+  if (c->batch > 1 && (c->force_path != FPM_FORCE_FUSED || c->np % 32 != 0)) return false;
   return true;
+}
+
+const size_t kSkew = (size_t)256 * (size_t)tune("SKEW256", 37);   // bytes between consecutive half-complex buffers
+
+inline int batch_of(const fpm_config& c) { return c.batch > 1 ? c.batch : 1; }
+
+// cached run graphs bake in the workspace pointers and the kernel selection: drop them when either changes
+void drop_graphs(fpm_ctx* ctx) {
+  for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+  ctx->graphs.clear();
 }
 
 // carved views of the caller's workspace
@@ -37,14 +52,20 @@ struct Workspace {
   float* F[3];
 };
 
+// every region holds `batch` meshes back to back; rho | F[0] | F[1] | F[2] stay contiguous (the interleaved
+// force mesh of the fused path, [batch][ng^3] float4, overlays them)
 Workspace carve(const fpm_ctx* ctx) {
   Workspace w;
   char* p = static_cast<char*>(ctx->ws);
   const int n = ctx->cfg.ng;
-  w.rho = reinterpret_cast<float*>(p); p += real_bytes(n);
-  for (int d = 0; d < 3; ++d) { w.F[d] = reinterpret_cast<float*>(p); p += real_bytes(n); }
-  w.dk = reinterpret_cast<float2*>(p); p += cplx_bytes(n);
-  for (int d = 0; d < 3; ++d) { w.fk[d] = reinterpret_cast<float2*>(p); p += cplx_bytes(n); }
+  const size_t b = (size_t)batch_of(ctx->cfg);
+  w.rho = reinterpret_cast<float*>(p); p += b * real_bytes(n);
+  for (int d = 0; d < 3; ++d) { w.F[d] = reinterpret_cast<float*>(p); p += b * real_bytes(n); }
+  // the four half-complex buffers are streamed concurrently at the same relative offset by the fused passes;
+  // their size is a large power of two times 17 or 33, so without a skew all streams fall on the same DRAM
+  // channels (measured: fft_z_c2r3 0.85 -> 1.02 ms with unskewed 128-byte-pitch buffers)
+  w.dk = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew;
+  for (int d = 0; d < 3; ++d) { w.fk[d] = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew; }
   return w;
 }
 
@@ -86,6 +107,8 @@ struct DeviceGuard {
   } while (0)
 #define FPM_REQUIRE(ctx, cond, what)                                \
   if (!(cond)) return fail((ctx), FPM_EINVAL, what);
+#define FPM_NO_BATCH(ctx, what)                                     \
+  if (batch_of((ctx)->cfg) > 1) return fail((ctx), FPM_ENOTIMPL, what ": not available on a batched context");
 #define FPM_NEED_WS(ctx)                                            \
   if (!(ctx)->ws || (ctx)->ws_bytes < fpm_workspace_bytes(&(ctx)->cfg)) \
     return fail((ctx), FPM_ENOMEM, "workspace missing or too small (fpm_set_workspace)");
@@ -110,10 +133,12 @@ int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, 
   const int ng = ctx->cfg.ng;
   cudaStream_t s = ctx->stream;
   Profiler* pr = &ctx->prof;
-  { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s)); }
+  const int batch = batch_of(ctx->cfg);
+  { ProfScope sc(pr, K_PAINT);
+    FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s, batch)); }
   if (ctx->cfg.force_path == FPM_FORCE_FUSED) {
     FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F,
-                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr));
+                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr, batch));
     return FPM_OK;
   }
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
@@ -135,7 +160,7 @@ int pm_step(fpm_ctx* ctx, const Workspace& w, float* pos, float* mom, int64_t n,
   ProfScope sc(&ctx->prof, K_READOUT_KICK_DRIFT);
   if (f4)
     FPM_CUDA(ctx, readout_kick_drift(w.rho, nullptr, nullptr, pos, mom, n, ctx->cfg.ng, (float)kfac,
-                                     (float)dfac, order_of(ctx, n), ctx->stream));
+                                     (float)dfac, order_of(ctx, n), ctx->stream, batch_of(ctx->cfg)));
   else
     FPM_CUDA(ctx, readout_kick_drift(w.F[0], w.F[1], w.F[2], pos, mom, n, ctx->cfg.ng, (float)kfac,
                                      (float)dfac, order_of(ctx, n), ctx->stream));
@@ -212,7 +237,7 @@ const char* fpm_version(void) { return "fpm-b200 0.1 (sm_100a)"; }
 
 size_t fpm_workspace_bytes(const fpm_config* cfg) {
   if (!config_ok(cfg)) return 0;
-  return 4 * real_bytes(cfg->ng) + 4 * cplx_bytes(cfg->ng);
+  return (size_t)batch_of(*cfg) * (4 * real_bytes(cfg->ng) + 4 * cplx_bytes(cfg->ng)) + 4 * kSkew;
 }
 
 int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
@@ -241,6 +266,8 @@ int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
 int fpm_destroy(fpm_ctx* ctx) {
   if (!ctx) return FPM_EINVAL;
   DeviceGuard device_guard__(ctx->device);
+  drop_graphs(ctx);
+  if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
   ctx->prof.destroy();
   if (ctx->d_acc) cudaFree(ctx->d_acc);
   fft_tables_destroy(&ctx->fft_g);
@@ -258,6 +285,7 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
   FPM_REQUIRE(ctx, ws != nullptr, "workspace is null");
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(ws) & 255) == 0, "workspace must be 256-byte aligned");
   if (bytes < fpm_workspace_bytes(&ctx->cfg)) return fail(ctx, FPM_ENOMEM, "workspace too small");
+  drop_graphs(ctx);
   ctx->ws = ws;
   ctx->ws_bytes = bytes;
   return FPM_OK;
@@ -266,7 +294,15 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
 int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode) {
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, paint_mode >= FPM_PAINT_AUTO && paint_mode <= FPM_PAINT_BRICK_FIXED, "unknown paint mode");
+  drop_graphs(ctx);
   ctx->cfg.paint_mode = paint_mode;
+  return FPM_OK;
+}
+
+int fpm_set_graph_mode(fpm_ctx* ctx, int graph_mode) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, graph_mode >= FPM_GRAPH_OFF && graph_mode <= FPM_GRAPH_ALWAYS, "unknown graph mode");
+  ctx->graph_mode = graph_mode;
   return FPM_OK;
 }
 
@@ -302,12 +338,14 @@ int fpm_paint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n, floa
   FPM_ENTER(ctx);
   FPM_REQUIRE(ctx, n >= 0 && mesh && (pos || n == 0), "fpm_paint: bad arguments");
   ProfScope sc(&ctx->prof, K_PAINT);
-  FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, order_of(ctx, n), ctx->stream));
+  FPM_CUDA(ctx, paint(pos, mass, particle_mass(ctx), n, ctx->cfg.ng, mesh, true, order_of(ctx, n), ctx->stream,
+                      batch_of(ctx->cfg)));
   return FPM_OK;
 }
 
 int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_fft_r2c");
   FPM_REQUIRE(ctx, real && cplx, "fpm_fft_r2c: null pointer");
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
               "fpm_fft_r2c: pointers must be 8-byte aligned");
@@ -317,6 +355,7 @@ int fpm_fft_r2c(fpm_ctx* ctx, const float* real, float* cplx) {
 
 int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_fft_c2r");
   FPM_REQUIRE(ctx, real && cplx, "fpm_fft_c2r: null pointer");
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(real) & 7) == 0 && (reinterpret_cast<uintptr_t>(cplx) & 7) == 0,
               "fpm_fft_c2r: pointers must be 8-byte aligned");
@@ -327,6 +366,7 @@ int fpm_fft_c2r(fpm_ctx* ctx, float* cplx, float* real) {
 int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, float* fkx, float* fky,
                            float* fkz) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_apply_force_kernel");
   FPM_REQUIRE(ctx, delta_k && fkx && fky && fkz, "fpm_apply_force_kernel: null pointer");
   FPM_REQUIRE(ctx, delta_k != fkx && delta_k != fky && delta_k != fkz,
               "fpm_apply_force_kernel: outputs must not alias the input");
@@ -339,6 +379,7 @@ int fpm_apply_force_kernel(fpm_ctx* ctx, const float* delta_k, float scale, floa
 
 int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, float* out) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_readout");
   FPM_REQUIRE(ctx, n >= 0 && mesh && ((pos && out) || n == 0), "fpm_readout: bad arguments");
   ProfScope sc(&ctx->prof, K_READOUT);
   FPM_CUDA(ctx, readout(mesh, pos, n, ctx->cfg.ng, out, order_of(ctx, n), ctx->stream));
@@ -347,6 +388,7 @@ int fpm_readout(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n, fl
 
 int fpm_force(fpm_ctx* ctx, const float* pos, int64_t n, float* force) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_force");
   FPM_REQUIRE(ctx, n >= 0 && ((pos && force) || n == 0), "fpm_force: bad arguments");
   FPM_NEED_WS(ctx);
   const Workspace w = carve(ctx);
@@ -384,6 +426,14 @@ int fpm_drift(fpm_ctx* ctx, float* pos, const float* mom, int64_t n, double ai, 
   return FPM_OK;
 }
 
+}  // extern "C"
+
+namespace {
+int lpt_init_one(fpm_ctx* ctx, const float* delta_lin, double a0, int order, float* pos, float* mom);
+}
+
+extern "C" {
+
 int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, float* pos,
                  float* mom) {
   FPM_ENTER(ctx);
@@ -391,6 +441,20 @@ int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, flo
   FPM_REQUIRE(ctx, order == 1 || order == 2, "fpm_lpt_init: order must be 1 or 2");
   FPM_REQUIRE(ctx, a0 > 0.0, "fpm_lpt_init: a0 must be positive");
   FPM_NEED_WS(ctx);
+  // initial conditions are made once per run: the simulations of a batch take their turn (Alg. 4 each)
+  const int64_t n3 = (int64_t)ctx->cfg.np * ctx->cfg.np * ctx->cfg.np;
+  for (int b = 0; b < batch_of(ctx->cfg); ++b) {
+    const int rc = lpt_init_one(ctx, delta_lin + b * n3, a0, order, pos + 3 * b * n3, mom + 3 * b * n3);
+    if (rc != FPM_OK) return rc;
+  }
+  return FPM_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+int lpt_init_one(fpm_ctx* ctx, const float* delta_lin, double a0, int order, float* pos, float* mom) {
   const Workspace w = carve(ctx);
   cudaStream_t s = ctx->stream;
   const int np = ctx->cfg.np, ng = ctx->cfg.ng, bfac = ng / np;
@@ -437,6 +501,77 @@ int fpm_lpt_init(fpm_ctx* ctx, const float* delta_lin, double a0, int order, flo
   return FPM_OK;
 }
 
+// the n_steps + 1 PM steps of a run, enqueued kernel by kernel on ctx->stream
+int run_steps(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& kf, const std::vector<double>& dr,
+              float* traj) {
+  const Workspace w = carve(ctx);
+  const int64_t n = (int64_t)ctx->cfg.np * ctx->cfg.np * ctx->cfg.np;
+  const size_t state = sizeof(float) * 3 * (size_t)n * batch_of(ctx->cfg);
+  for (size_t j = 0; j < kf.size(); ++j) {
+    if (traj)
+      FPM_CUDA(ctx, cudaMemcpyAsync(reinterpret_cast<char*>(traj) + j * state, pos, state, cudaMemcpyDeviceToDevice,
+                                    ctx->stream));
+    const int rc = pm_step(ctx, w, pos, mom, n, kf[j], dr[j]);
+    if (rc != FPM_OK) return rc;
+  }
+  return FPM_OK;
+}
+
+// The same run as ONE CUDA graph launch (fpm.h FPM_GRAPH_*): a small configuration spends its step in launch
+// latency (C1: 8 launches of 6-24 us for 0.1 ms of work), so the run is captured once -- on an internal stream:
+// the caller's may be the legacy default stream, which cannot be captured -- and replayed on ctx->stream.
+// Graphs are cached per (pos, mom, traj, factors).  Returns FPM_ENOTIMPL when capture is not possible (the
+// caller then enqueues kernel by kernel); nothing has been enqueued in that case.
+int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& kf, const std::vector<double>& dr,
+              float* traj) {
+  for (auto& g : ctx->graphs)
+    if (g.pos == pos && g.mom == mom && g.traj == traj && g.kf == kf && g.dr == dr) {
+      FPM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+      ctx->prof.launches += g.launches;
+      return FPM_OK;
+    }
+  if (!ctx->capture_stream &&
+      cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    return FPM_ENOTIMPL;
+  }
+  cudaStream_t user = ctx->stream;
+  const long long before = ctx->prof.launches;
+  if (cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+    cudaGetLastError();
+    return FPM_ENOTIMPL;
+  }
+  ctx->stream = ctx->capture_stream;
+  ctx->prof.stream = ctx->capture_stream;
+  const int rc = run_steps(ctx, pos, mom, kf, dr, traj);
+  ctx->stream = user;
+  ctx->prof.stream = user;
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(ctx->capture_stream, &graph);
+  const long long nodes = ctx->prof.launches - before;
+  ctx->prof.launches = before;
+  cudaGraphExec_t exec = nullptr;
+  if (rc != FPM_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    ctx->sticky = false;                 // a failed capture enqueued nothing; the eager path reports real errors
+    return FPM_ENOTIMPL;
+  }
+  cudaGraphDestroy(graph);
+  if (ctx->graphs.size() >= 8) {         // small cache: drop the oldest
+    cudaGraphExecDestroy(ctx->graphs.front().exec);
+    ctx->graphs.erase(ctx->graphs.begin());
+  }
+  ctx->graphs.push_back(fpm_ctx::RunGraph{pos, mom, traj, kf, dr, exec, nodes});
+  FPM_CUDA(ctx, cudaGraphLaunch(exec, ctx->stream));
+  ctx->prof.launches += nodes;
+  return FPM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int n_steps,
               float* traj) {
   FPM_ENTER(ctx);
@@ -444,25 +579,22 @@ int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int 
   for (int j = 0; j <= n_steps; ++j)
     FPM_REQUIRE(ctx, a_stages[j] > 0.0, "fpm_nbody: scale factors must be positive");
   FPM_NEED_WS(ctx);
-  const Workspace w = carve(ctx);
-  cudaStream_t s = ctx->stream;
-  const int np = ctx->cfg.np;
-  const int64_t n = (int64_t)np * np * np;
   std::vector<double> kf(n_steps + 1), dr(n_steps + 1);
   step_factors(ctx, a_stages, n_steps, kf.data(), dr.data());
-  for (int j = 0; j <= n_steps; ++j) {
-    if (traj)
-      FPM_CUDA(ctx, cudaMemcpyAsync(traj + (int64_t)j * 3 * n, pos, sizeof(float) * 3 * n,
-                                    cudaMemcpyDeviceToDevice, s));
-    const int rc = pm_step(ctx, w, pos, mom, n, kf[j], dr[j]);
-    if (rc != FPM_OK) return rc;
+  const int64_t cells = (int64_t)batch_of(ctx->cfg) * ctx->cfg.ng * ctx->cfg.ng * ctx->cfg.ng;
+  const bool want_graph = ctx->graph_mode == FPM_GRAPH_ALWAYS ||
+                          (ctx->graph_mode == FPM_GRAPH_AUTO && cells <= (int64_t(1) << 24));
+  if (want_graph && !ctx->prof.enabled) {          // (per-kernel event timing needs the kernel-by-kernel path)
+    const int rc = run_graph(ctx, pos, mom, kf, dr, traj);
+    if (rc != FPM_ENOTIMPL) return rc;
   }
-  return FPM_OK;
+  return run_steps(ctx, pos, mom, kf, dr, traj);
 }
 
 int fpm_nbody_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom,
                    const double* a_stages, int n_steps) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_nbody_host");
   FPM_REQUIRE(ctx, h_pos && h_mom && d_pos && d_mom, "fpm_nbody_host: null pointer");
   const int64_t n = (int64_t)ctx->cfg.np * ctx->cfg.np * ctx->cfg.np;
   const size_t bytes = sizeof(float) * 3 * (size_t)n;
@@ -488,6 +620,7 @@ int fpm_pm_step(fpm_ctx* ctx, float* pos, float* mom, int64_t n, double kick_fac
 int fpm_pm_step_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, float* d_mom, int64_t n,
                      double kick_fac, double drift_fac) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_pm_step_host");
   FPM_REQUIRE(ctx, n >= 0 && h_pos && h_mom && d_pos && d_mom, "fpm_pm_step_host: bad arguments");
   const size_t bytes = sizeof(float) * 3 * (size_t)n;
   cudaStream_t s = ctx->stream;
@@ -504,6 +637,7 @@ int fpm_pm_step_host(fpm_ctx* ctx, float* h_pos, float* h_mom, float* d_pos, flo
 int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, double coef,
                   float* grad_pos) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_force_vjp");
   FPM_REQUIRE(ctx, n >= 0 && ((pos && v && grad_pos) || n == 0), "fpm_force_vjp: bad arguments");
   FPM_REQUIRE(ctx, std::isfinite(coef), "fpm_force_vjp: non-finite coefficient");
   FPM_NEED_WS(ctx);
@@ -513,6 +647,7 @@ int fpm_force_vjp(fpm_ctx* ctx, const float* pos, int64_t n, const float* v, dou
 int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n_steps,
                   float* grad_pos, float* grad_mom, int flags) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_nbody_vjp");
   FPM_REQUIRE(ctx, traj && a_stages && grad_pos && grad_mom && n_steps >= 0, "fpm_nbody_vjp: bad arguments");
   FPM_REQUIRE(ctx, (flags & ~FPM_VJP_GRAD_MOM_ZERO) == 0, "fpm_nbody_vjp: unknown flag");
   for (int j = 0; j <= n_steps; ++j)
@@ -544,6 +679,7 @@ int fpm_nbody_vjp(fpm_ctx* ctx, const float* traj, const double* a_stages, int n
 int fpm_lpt_init_vjp(fpm_ctx* ctx, const float* delta_lin, double a0, int order,
                      const float* grad_pos, const float* grad_mom, float* grad_delta) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_lpt_init_vjp");
   FPM_REQUIRE(ctx, delta_lin && grad_pos && grad_mom && grad_delta, "fpm_lpt_init_vjp: null pointer");
   FPM_REQUIRE(ctx, order == 1 || order == 2, "fpm_lpt_init_vjp: order must be 1 or 2");
   FPM_REQUIRE(ctx, a0 > 0.0, "fpm_lpt_init_vjp: a0 must be positive");
@@ -619,6 +755,7 @@ int fpm_recon_loss_grad(fpm_ctx* ctx, const float* s_lin, const float* data, dou
                         const float* inv_power, const double* a_stages, int n_steps, int lpt_order,
                         void* scratch, size_t scratch_bytes, float* grad, double* loss) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_recon_loss_grad");
   FPM_REQUIRE(ctx, s_lin && data && inv_power && a_stages && scratch && grad && loss && n_steps >= 0,
               "fpm_recon_loss_grad: bad arguments");
   FPM_REQUIRE(ctx, sigma > 0.0, "fpm_recon_loss_grad: sigma must be positive");
@@ -709,6 +846,7 @@ int64_t fpm_launch_count(const fpm_ctx* ctx) { return ctx ? ctx->prof.launches :
 int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t n,
                       const float* grad_mesh, float* grad_pos, float* grad_mass) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_paint_adjoint");
   FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_pos) || n == 0), "fpm_paint_adjoint: bad arguments");
   ProfScope sc(&ctx->prof, K_READOUT_GRAD);
   FPM_CUDA(ctx, readout_grad(grad_mesh, pos, mass, particle_mass(ctx), n, ctx->cfg.ng, grad_pos,
@@ -719,6 +857,7 @@ int fpm_paint_adjoint(fpm_ctx* ctx, const float* pos, const float* mass, int64_t
 int fpm_readout_adjoint(fpm_ctx* ctx, const float* mesh, const float* pos, int64_t n,
                         const float* grad_out, float* grad_mesh, float* grad_pos) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_readout_adjoint");
   FPM_REQUIRE(ctx, n >= 0 && grad_mesh && ((pos && grad_out) || n == 0), "fpm_readout_adjoint: bad arguments");
   FPM_REQUIRE(ctx, !grad_pos || mesh, "fpm_readout_adjoint: grad_pos needs the forward mesh");
   { ProfScope sc(&ctx->prof, K_PAINT); FPM_CUDA(ctx, paint(pos, grad_out, 0.f, n, ctx->cfg.ng, grad_mesh, false, order_of(ctx, n), ctx->stream)); }

@@ -76,7 +76,7 @@ cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaSt
     auto kern = fft_z_r2c_kernel<N>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(real, cplx, nrows, t.stage_m, t.full);
+    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(real, cplx, nrows, t.stage_m, t.full, nzh);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
@@ -94,7 +94,7 @@ cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaSt
 
 template <int N>
 cudaError_t launch_z_c2r(const FftTables& t, const float2* cplx, float* real, const float* gz,
-                         cudaStream_t s, Profiler* prof) {
+                         cudaStream_t s, Profiler* prof, int pitch = N / 2 + 1) {
   constexpr int M = N / 2, G = z_rows<N>();
   const int64_t nrows = (int64_t)N * N;
   ProfScope sc(prof, K_FFT_Z_C2R);
@@ -104,7 +104,7 @@ cudaError_t launch_z_c2r(const FftTables& t, const float2* cplx, float* real, co
   cudaError_t e = set_smem(kern, smem);
   if (e != cudaSuccess) return e;
   const float scale = (float)(1.0 / ((double)N * N * N));
-  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz);
+  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz, pitch);
   return cudaGetLastError();
 }
 
@@ -129,56 +129,89 @@ cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t
 // function (one forward, two inverse transforms per column), 3 inverse y passes in one launch, then
 // either 3 planar c2r z passes into F[0..2] or, when F4 is given, one launch writing the interleaved
 // (F_x, F_y, F_z, 0) mesh (g(w_z) fused into the z pass of the third component either way).
-// wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.
+// wa, wb, wc: three half-complex scratch buffers; dk is both input scratch and Fy scratch.  All four are
+// internal, with the padded row pitch PZ = padded_pitch(N) (128-byte aligned rows and 16-column tiles).
+template <int N>
+cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, const float2* in, float2* out_a,
+                                float2* out_bx, float scale, bool poisson, cudaStream_t s, int batch = 1) {
+  constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N), TX = xf_tile<N>();
+  const dim3 grid((nzh + TX - 1) / TX, N, batch);
+  const unsigned threads = TX * Plan<N, xf_variant<N>()>::P;
+  cudaError_t e;
+  auto go = [&](auto kern) -> cudaError_t {
+    e = set_smem(kern, xf_smem_bytes<N>());
+    if (e != cudaSuccess) return e;
+    kern<<<grid, threads, xf_smem_bytes<N>(), s>>>(in, out_a, poisson ? nullptr : out_bx, nzh, PZ, t.stage_x, kt.lap,
+                                                   kt.grad, scale);
+    return cudaGetLastError();
+  };
+  if (tune("XSWZ", 0) && TX == 8)
+    return poisson ? go(fft_x_force_kernel<N, true, true>) : go(fft_x_force_kernel<N, false, true>);
+  return poisson ? go(fft_x_force_kernel<N, true, false>) : go(fft_x_force_kernel<N, false, false>);
+}
+
+template <int N>
+cudaError_t launch_z_r2c_padded(const FftTables& t, const float* real, float2* cplx, cudaStream_t s, int batch = 1) {
+  constexpr int M = N / 2, G = z_rows<N>(), PZ = padded_pitch(N);
+  const int64_t nrows = (int64_t)N * N * batch;      // rows of consecutive meshes are consecutive
+  constexpr int threads = G * Plan<M>::P;
+  const size_t smem = sizeof(float2) * G * row_pitch(M);
+  auto kern = fft_z_r2c_kernel<N>;
+  cudaError_t e = set_smem(kern, smem);
+  if (e != cudaSuccess) return e;
+  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(real, cplx, nrows, t.stage_m, t.full, PZ);
+  return cudaGetLastError();
+}
+
 template <int N>
 cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                              float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                             cudaStream_t s, Profiler* prof) {
-  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>(), T = col_tile<N>();
-  const int64_t nrows = (int64_t)N * N;
+                             cudaStream_t s, Profiler* prof, int batch) {
+  constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N);
+  // a batch of meshes back to back: its z rows and its x slabs are just more rows / slabs; only the x
+  // round trip, whose lines stride across a whole mesh, takes the mesh index as a grid dimension
+  if (batch < 1 || (batch > 1 && !F4) || (int64_t)N * batch > 65535) return cudaErrorInvalidValue;
+  const int64_t nrows = (int64_t)N * N * batch;
+  const int slabs = N * batch;
   cudaError_t e;
   {
     ProfScope sc(prof, K_FFT_Z_R2C);
-    constexpr int threads = G * Plan<M>::P;
-    const size_t smem = sizeof(float2) * G * row_pitch(M);
-    auto kern = fft_z_r2c_kernel<N>;
-    e = set_smem(kern, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(rho, dk, nrows, t.stage_m, t.full);
-    e = cudaGetLastError();
+    e = launch_z_r2c_padded<N>(t, rho, dk, s, batch);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    e = launch_cols<N, false>(dk, dk, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    e = launch_cols<N, false>(dk, dk, slabs, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
     if (e != cudaSuccess) return e;
   }
-  constexpr int threads = T * Plan<N>::P;
-  const size_t smem = Plan<N>::NST > 1 ? sizeof(float2) * N * T : 0;
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
-    constexpr int TX = xf_tile<N>();
-    auto kern = fft_x_force_kernel<N>;
-    e = set_smem(kern, xf_smem_bytes<N>());
-    if (e != cudaSuccess) return e;
-    const int ncols = N * nzh;
-    kern<<<(ncols + TX - 1) / TX, TX * Plan<N, xf_variant<N>()>::P, xf_smem_bytes<N>(), s>>>(
-        dk, wa, wb, ncols, nzh, (int64_t)N * nzh, t.stage_x, kt.lap, kt.grad, scale);
-    e = cudaGetLastError();
+    e = launch_x_round_trip<N>(t, kt, dk, wa, wb, scale, false, s, batch);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_Y_INV3);
     using YPL = Plan<N, yi_variant<N>()>;
-    constexpr int TY = yi_tile<N>();
-    const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
-    auto kern = fft_y_inv3_kernel<N>;
-    e = set_smem(kern, ysmem);
-    if (e != cudaSuccess) return e;
-    dim3 grid(3 * ((nzh + TY - 1) / TY), N);
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    kern<<<grid, TY * YPL::P, ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * nzh, nzh, nzh,
-                                         yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+    if (tune("YPAIR", 1)) {
+      constexpr int TY = yi_tile<N>();
+      const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
+      auto kern = fft_y_inv3_pair_kernel<N>;
+      e = set_smem(kern, ysmem);
+      if (e != cudaSuccess) return e;
+      dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
+      kern<<<grid, yi_threads<N>(), ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * PZ, nzh, PZ,
+                                                yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+    } else {
+      constexpr int TY = yi1_tile<N>();
+      const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
+      auto kern = fft_y_inv3_kernel<N>;
+      e = set_smem(kern, ysmem);
+      if (e != cudaSuccess) return e;
+      dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
+      kern<<<grid, TY * YPL::P, ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * PZ, nzh, PZ,
+                                            yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
@@ -186,63 +219,51 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     ProfScope sc(prof, K_FFT_Z_C2R3);
     constexpr int GC = z3_rows<N>();
     const size_t zsmem = z3_smem_bytes<N>();
-    auto kern = fft_z_c2r3_kernel<N>;
-    e = set_smem(kern, zsmem);
-    if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((nrows + GC - 1) / GC), z3_threads<N>(), zsmem, s>>>(
-        wb, dk, wc, reinterpret_cast<float4*>(F4), nrows, t.stage_m, t.full,
-        (float)(1.0 / ((double)N * N * N)), kt.grad);
-    return cudaGetLastError();
+    auto go = [&](auto kern) -> cudaError_t {
+      e = set_smem(kern, zsmem);
+      if (e != cudaSuccess) return e;
+      kern<<<(unsigned)((nrows + GC - 1) / GC), z3_threads<N>(), zsmem, s>>>(
+          wb, dk, wc, reinterpret_cast<float4*>(F4), nrows, t.stage_m, t.full,
+          (float)(1.0 / ((double)N * N * N)), kt.grad);
+      return cudaGetLastError();
+    };
+    return tune("ZTMA", 1) ? go(fft_z_c2r3_kernel<N, true>) : go(fft_z_c2r3_kernel<N, false>);
   }
-  e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof);
+  e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof, PZ);
   if (e != cudaSuccess) return e;
-  e = launch_z_c2r<N>(t, dk, F[1], nullptr, s, prof);
+  e = launch_z_c2r<N>(t, dk, F[1], nullptr, s, prof, PZ);
   if (e != cudaSuccess) return e;
-  return launch_z_c2r<N>(t, wc, F[2], kt.grad, s, prof);
+  return launch_z_c2r<N>(t, wc, F[2], kt.grad, s, prof, PZ);
 }
 
 // real mesh -> real mesh:  out = c2r[ (scale / K^2) r2c[src] ]  (K^2 of the context's kernel mode, 0 at k = 0),
-// with the multiplier fused into the x round trip; work: one half-complex scratch buffer.
+// with the multiplier fused into the x round trip; work: one half-complex scratch buffer (padded pitch).
 template <int N>
 cudaError_t poisson_impl(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
                          float scale, cudaStream_t s, Profiler* prof) {
-  constexpr int M = N / 2, nzh = M + 1, G = z_rows<N>();
-  const int64_t nrows = (int64_t)N * N;
+  constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N);
   cudaError_t e;
   {
     ProfScope sc(prof, K_FFT_Z_R2C);
-    constexpr int threads = G * Plan<M>::P;
-    const size_t smem = sizeof(float2) * G * row_pitch(M);
-    auto kern = fft_z_r2c_kernel<N>;
-    e = set_smem(kern, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(src, work, nrows, t.stage_m, t.full);
-    e = cudaGetLastError();
+    e = launch_z_r2c_padded<N>(t, src, work, s);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    e = launch_cols<N, false>(work, work, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    e = launch_cols<N, false>(work, work, N, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
-    constexpr int TX = xf_tile<N>();
-    auto kern = fft_x_force_kernel<N, true>;
-    e = set_smem(kern, xf_smem_bytes<N>());
-    if (e != cudaSuccess) return e;
-    const int ncols = N * nzh;
-    kern<<<(ncols + TX - 1) / TX, TX * Plan<N, xf_variant<N>()>::P, xf_smem_bytes<N>(), s>>>(
-        work, work, nullptr, ncols, nzh, (int64_t)N * nzh, t.stage_x, kt.lap, kt.grad, scale);
-    e = cudaGetLastError();
+    e = launch_x_round_trip<N>(t, kt, work, work, nullptr, scale, true, s);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    e = launch_cols<N, true>(work, work, N, (int64_t)N * nzh, nzh, nzh, t.stage_n, s);
+    e = launch_cols<N, true>(work, work, N, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
     if (e != cudaSuccess) return e;
   }
-  return launch_z_c2r<N>(t, work, out, nullptr, s, prof);
+  return launch_z_c2r<N>(t, work, out, nullptr, s, prof, PZ);
 }
 
 }  // namespace
@@ -309,9 +330,9 @@ cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float*
 
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof) {
+                            cudaStream_t s, Profiler* prof, int batch) {
   if (kt.n != t.n) return cudaErrorInvalidValue;
-  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof)
+  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof, batch)
 }
 
 }  // namespace fpm

@@ -30,6 +30,16 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 }
 __device__ __forceinline__ float2 cswap(float2 a) { return make_float2(a.y, a.x); }
 
+// The same line position of two ADJACENT columns, transformed together by one thread: a column pass that
+// moves 16 bytes per lane touches half as many 128-byte lines per request as one that moves 8 (the L1 data
+// pipe, not DRAM, bounded the 8-byte column passes: profiles/r01_E_C4.md), and the two independent
+// butterflies give the scheduler twice the instruction-level parallelism.
+struct cpair { float2 a, b; };
+__device__ __forceinline__ cpair cadd(cpair x, cpair y) { return cpair{cadd(x.a, y.a), cadd(x.b, y.b)}; }
+__device__ __forceinline__ cpair csub(cpair x, cpair y) { return cpair{csub(x.a, y.a), csub(x.b, y.b)}; }
+__device__ __forceinline__ cpair cmul(cpair x, float2 w) { return cpair{cmul(x.a, w), cmul(x.b, w)}; }
+__device__ __forceinline__ cpair cswap(cpair x) { return cpair{cswap(x.a), cswap(x.b)}; }
+
 // cos(2 pi k / 32), k = 0..8
 __host__ __device__ constexpr float cos32_table(int k) {
   constexpr float c[9] = {1.0f,
@@ -52,6 +62,10 @@ __host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
 
 // x * exp(-2 pi i I / R), resolved at compile time
 template <int R, int I>
+__device__ __forceinline__ float2 mul_twiddle(float2 x);
+template <int R, int I>
+__device__ __forceinline__ cpair mul_twiddle(cpair x) { return cpair{mul_twiddle<R, I>(x.a), mul_twiddle<R, I>(x.b)}; }
+template <int R, int I>
 __device__ __forceinline__ float2 mul_twiddle(float2 x) {
   constexpr int k = (I * (32 / R)) % 32;
   if constexpr (k == 0) return x;
@@ -65,28 +79,32 @@ __device__ __forceinline__ float2 mul_twiddle(float2 x) {
 }
 
 // In-register forward DFT of R points (decimation in frequency), natural-order output.
+// (C = float2, or cpair: two columns at once)
 template <int R>
 struct Dft {
-  template <int... I>
-  static __device__ __forceinline__ void run(float2 (&v)[R], std::integer_sequence<int, I...>) {
-    float2 e[R / 2], o[R / 2];
+  template <class C, int... I>
+  static __device__ __forceinline__ void run(C (&v)[R], std::integer_sequence<int, I...>) {
+    C e[R / 2], o[R / 2];
     ((e[I] = cadd(v[I], v[I + R / 2]), o[I] = mul_twiddle<R, I>(csub(v[I], v[I + R / 2]))), ...);
     Dft<R / 2>::apply(e);
     Dft<R / 2>::apply(o);
     ((v[2 * I] = e[I], v[2 * I + 1] = o[I]), ...);
   }
-  static __device__ __forceinline__ void apply(float2 (&v)[R]) {
+  template <class C>
+  static __device__ __forceinline__ void apply(C (&v)[R]) {
     run(v, std::make_integer_sequence<int, R / 2>{});
   }
 };
 template <>
 struct Dft<1> {
-  static __device__ __forceinline__ void apply(float2 (&)[1]) {}
+  template <class C>
+  static __device__ __forceinline__ void apply(C (&)[1]) {}
 };
 template <>
 struct Dft<2> {
-  static __device__ __forceinline__ void apply(float2 (&v)[2]) {
-    const float2 a = v[0], b = v[1];
+  template <class C>
+  static __device__ __forceinline__ void apply(C (&v)[2]) {
+    const C a = v[0], b = v[1];
     v[0] = cadd(a, b);
     v[1] = csub(a, b);
   }
@@ -129,13 +147,29 @@ FPM_PLAN_V(512, 1, 8, 3, 8, 8, 8)
 #undef FPM_PLAN_V
 
 // shared-memory accessors -----------------------------------------------------------------
-// column tile: element i of column c at i*T + c (lanes run over c: conflict-free)
-template <int T>
+// column tile: element i of column c at i*T + c.  With T = 16 a line of the tile is 128 bytes, all 32 banks:
+// conflict-free by construction.  With T = 8 a line is 64 bytes, half the banks, and the two lines a
+// half-warp touches must fall in different halves; the line index is therefore XOR-swizzled with the parity
+// of its upper bits, which separates any two lines whose indices differ in exactly one bit (every access
+// pattern of the Stockham stages: consecutive lines, or lines a power-of-two stride apart).
+template <int T, bool SWZ = false>
 struct ColSmem {
   float2* base;
   int c;
-  __device__ __forceinline__ void st(int i, float2 x) const { base[i * T + c] = x; }
-  __device__ __forceinline__ float2 ld(int i) const { return base[i * T + c]; }
+  __device__ __forceinline__ static int line(int i) { return (T == 8 && SWZ) ? (i ^ (__popc(i >> 1) & 1)) : i; }
+  __device__ __forceinline__ void st(int i, float2 x) const { base[line(i) * T + c] = x; }
+  __device__ __forceinline__ float2 ld(int i) const { return base[line(i) * T + c]; }
+};
+// the same tile accessed as column pairs: pair c2 of line i is one 16-byte word (T = 16: a line is 128 bytes)
+template <int T>
+struct ColSmem2 {
+  float4* base;
+  int c2;
+  __device__ __forceinline__ void st(int i, cpair x) const { base[i * (T / 2) + c2] = make_float4(x.a.x, x.a.y, x.b.x, x.b.y); }
+  __device__ __forceinline__ cpair ld(int i) const {
+    const float4 q = base[i * (T / 2) + c2];
+    return cpair{make_float2(q.x, q.y), make_float2(q.z, q.w)};
+  }
 };
 // contiguous line: lanes run over the butterfly index; one pad slot per 16 breaks stride-R conflicts
 struct RowSmem {
@@ -150,8 +184,8 @@ __host__ __device__ constexpr int row_pitch(int m) { return m + (m >> 4) + 1; }
 // Stage with radix R, NS lines already combined: butterfly j reads x[j + t N/R], multiplies by
 // exp(-2 pi i t k/(NS R)), k = j mod NS, and writes y[(j-k) R + k + t NS].
 // ------------------------------------------------------------------------------------------
-template <class PL, int S, class SM>
-__device__ __forceinline__ void fft_stage(float2 (&v)[PL::E], const int p, const SM& sm,
+template <class PL, int S, class SM, class C>
+__device__ __forceinline__ void fft_stage(C (&v)[PL::E], const int p, const SM& sm,
                                           const float2* __restrict__ tw) {
   constexpr int E = PL::E, P = PL::P, R = PL::radix(S), NS = PL::ns(S), M = E / R;
   constexpr bool last = (S == PL::NST - 1);
@@ -159,7 +193,7 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[PL::E], const int p, const
   for (int u = 0; u < M; ++u) {
     const int j = p + u * P;
     const int k = j & (NS - 1);
-    float2 a[R];
+    C a[R];
 #pragma unroll
     for (int t = 0; t < R; ++t) a[t] = v[u + t * M];
     if constexpr (NS > 1) {
@@ -182,7 +216,7 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[PL::E], const int p, const
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = sm.ld(p + P * e);
     if constexpr (S + 1 < PL::NST - 1) __syncthreads();
-    fft_stage<PL, S + 1, SM>(v, p, sm, tw);
+    fft_stage<PL, S + 1, SM, C>(v, p, sm, tw);
   }
 }
 
@@ -190,13 +224,18 @@ __device__ __forceinline__ void fft_stage(float2 (&v)[PL::E], const int p, const
 template <int N, class SM>
 __device__ __forceinline__ void fft_line(float2 (&v)[Plan<N>::E], const int p, const SM& sm,
                                          const float2* __restrict__ tw) {
-  fft_stage<Plan<N>, 0, SM>(v, p, sm, tw);
+  fft_stage<Plan<N>, 0, SM, float2>(v, p, sm, tw);
 }
 // the same with an explicit plan (tw must be that plan's stage table)
-template <class PL, class SM>
-__device__ __forceinline__ void fft_line_plan(float2 (&v)[PL::E], const int p, const SM& sm,
+template <class PL, class SM, class C>
+__device__ __forceinline__ void fft_line_plan(C (&v)[PL::E], const int p, const SM& sm,
                                               const float2* __restrict__ tw) {
-  fft_stage<PL, 0, SM>(v, p, sm, tw);
+  fft_stage<PL, 0, SM, C>(v, p, sm, tw);
 }
+
+// row pitch (in complex elements) of the library's INTERNAL half-complex meshes: n/2 + 1 rounded up to 16
+// elements = 128 bytes, so every row and every 16-column tile starts on a 128-byte line and column pairs are
+// 16-byte aligned.  Buffers that cross the C-ABI keep the dense pitch n/2 + 1 (the cuFFT r2c layout).
+__host__ __device__ constexpr int padded_pitch(int n) { return (n / 2 + 1 + 15) & ~15; }
 
 }  // namespace fpm

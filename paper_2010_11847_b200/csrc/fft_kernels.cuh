@@ -76,32 +76,35 @@ template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
 
 // POISSON: only  out_a = inverse_x[ (scale / K^2) forward_x[in] ]  (real multiplier, no gradient variant;
 // out_a may alias in) -- the x round trip of the backward pass's single potential solve.
-template <int N, bool POISSON = false>
-__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P)
+// grid = (ceil(nzh / T), N, batch): block (bx, y, b) owns the T columns kz = bx T .. of row y of mesh b;
+// element (x, y, kz) of a mesh at (x N + y) pitch + kz.
+template <int N, bool POISSON = false, bool SWZ = false>
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
 fft_x_force_kernel(const float2* in, float2* out_a,
-                   float2* __restrict__ out_bx, int ncols, int nzh, int64_t line_stride,
+                   float2* __restrict__ out_bx, int nzh, int pitch,
                    const float2* __restrict__ tw, const float* __restrict__ lap,
                    const float* __restrict__ grad, float scale) {
   extern __shared__ float2 smem[];
   using PL = Plan<N, xf_variant<N>()>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
-  const int64_t col = (int64_t)blockIdx.x * T + c;
-  const bool ok = col < ncols;
+  const int y = blockIdx.y, kz = blockIdx.x * T + c;
+  const bool ok = kz < nzh;
+  // blockIdx.z: mesh of a batch (meshes back to back)
+  const int64_t line_stride = (int64_t)N * pitch, col = (int64_t)blockIdx.z * N * line_stride + (int64_t)y * pitch + kz;
   float2 v[E];
 #pragma unroll
   for (int e = 0; e < E; ++e)
     v[e] = ok ? in[col + (int64_t)(p + P * e) * line_stride] : make_float2(0.f, 0.f);
-  ColSmem<T> sm{smem, c};
+  ColSmem<T, SWZ> sm{smem, c};
   fft_line_plan<PL>(v, p, sm, tw);
-  const int y = ok ? (int)(col / nzh) : 0, kz = ok ? (int)(col % nzh) : 0;
-  const float lyz = __ldg(lap + y) + __ldg(lap + kz);
+  const float lyz = __ldg(lap + y) + __ldg(lap + (ok ? kz : 0));
   float2* park = smem + N * T + threadIdx.x;          // element e of this thread at park[e * T * P]
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int i = p + P * e;
     const float k2 = __ldg(lap + i) + lyz;
-    const float f = (col == 0 && i == 0) ? 0.f : scale / k2;
+    const float f = ((y | kz | i) == 0) ? 0.f : scale / k2;
     if constexpr (POISSON) {
       v[e] = make_float2(v[e].y * f, v[e].x * f);        // f v, (im, re)-swapped
     } else {
@@ -134,18 +137,60 @@ fft_x_force_kernel(const float2* in, float2* out_a,
 // The three inverse y passes of the fused force path in one launch.  Block b: tile b / 3 of x slab
 // blockIdx.y, variant b % 3:  0: Bx -> Fx (in place),  1: g(w_y) A -> Fy,  2: A -> Fz (g(w_z) is applied
 // by the z pass).  in0/out0 may alias; A is read by variants 1 and 2 and written by neither.
-template <int N> __host__ __device__ constexpr int yi_tile() { return N == 512 ? 8 : col_tile<N>(); }
+// A thread transforms a PAIR of adjacent columns (cpair): every global and shared access is 16 bytes per
+// lane, a tile line is 16 columns = one 128-byte line (the meshes have the padded pitch, a multiple of 16).
+// At N >= 512 it runs the 8-points-per-thread plan (16 complex values per thread for the pair).
+template <int N> __host__ __device__ constexpr int yi_tile() { return 16; }
 template <int N> __host__ __device__ constexpr int yi_variant() { return N == 512 ? 1 : 0; }
+template <int N> __host__ __device__ constexpr int yi_threads() { return (yi_tile<N>() / 2) * Plan<N, yi_variant<N>()>::P; }
 
 template <int N>
-__global__ void __launch_bounds__(yi_tile<N>() * Plan<N, yi_variant<N>()>::P)
-fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
+__global__ void __launch_bounds__(yi_threads<N>())
+fft_y_inv3_pair_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
                   float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
                   int ncols, int64_t line_stride, const float2* __restrict__ tw,
                   const float* __restrict__ grad) {
   extern __shared__ float2 smem[];
   using PL = Plan<N, yi_variant<N>()>;
   constexpr int T = yi_tile<N>(), E = PL::E, P = PL::P;
+  const int c2 = threadIdx.x % (T / 2), p = threadIdx.x / (T / 2);
+  const int variant = blockIdx.x % 3;
+  const int col = (blockIdx.x / 3) * T + 2 * c2;        // first column of the pair (the pitch is even)
+  const bool ok = col < ncols;                          // a pair may hold one pad column: computed, never used
+  const int64_t off = (int64_t)blockIdx.y * batch_stride + col;
+  const float2* in = variant == 0 ? in_bx : in_a;
+  float2* out = variant == 0 ? out_x : (variant == 1 ? out_y : out_z);
+  cpair v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (ok) q = *reinterpret_cast<const float4*>(in + off + (int64_t)i * line_stride);
+    if (variant == 1) { const float g = __ldg(grad + i); q.x *= g; q.y *= g; q.z *= g; q.w *= g; }
+    v[e] = cpair{make_float2(q.y, q.x), make_float2(q.w, q.z)};     // (im, re)-swapped: inverse transform
+  }
+  ColSmem2<T> sm{reinterpret_cast<float4*>(smem), c2};
+  fft_line_plan<PL>(v, p, sm, tw);
+  if (ok) {
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+      *reinterpret_cast<float4*>(out + off + (int64_t)(p + P * e) * line_stride) =
+          make_float4(v[e].a.y, v[e].a.x, v[e].b.y, v[e].b.x);
+  }
+}
+
+// the same pass with one column per thread (8-byte accesses; 8-column tiles at N = 512)
+template <int N> __host__ __device__ constexpr int yi1_tile() { return N == 512 ? 8 : col_tile<N>(); }
+
+template <int N>
+__global__ void __launch_bounds__(yi1_tile<N>() * Plan<N, yi_variant<N>()>::P)
+fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
+                  float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
+                  int ncols, int64_t line_stride, const float2* __restrict__ tw,
+                  const float* __restrict__ grad) {
+  extern __shared__ float2 smem[];
+  using PL = Plan<N, yi_variant<N>()>;
+  constexpr int T = yi1_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
   const int variant = blockIdx.x % 3;
   const int64_t col = (int64_t)(blockIdx.x / 3) * T + c;
@@ -162,7 +207,7 @@ fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* 
     if (variant == 1) { const float g = __ldg(grad + i); x.x *= g; x.y *= g; }
     v[e] = cswap(x);
   }
-  ColSmem<T> sm{smem, c};
+  ColSmem<T, true> sm{smem, c};
   fft_line_plan<PL>(v, p, sm, tw);
   if (ok) {
 #pragma unroll
@@ -174,7 +219,7 @@ fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* 
 template <int N>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
 fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t nrows,
-                 const float2* __restrict__ tw, const float2* __restrict__ twn) {
+                 const float2* __restrict__ tw, const float2* __restrict__ twn, int out_pitch) {
   extern __shared__ float2 smem[];
   constexpr int M = N / 2;
   using PL = Plan<M>;
@@ -193,7 +238,7 @@ fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t
   for (int e = 0; e < E; ++e) sm.st(p + P * e, v[e]);
   __syncthreads();
   if (!ok) return;
-  float2* dst = out + row * (M + 1);
+  float2* dst = out + row * out_pitch;
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int k = p + P * e;
@@ -217,7 +262,7 @@ template <int N>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
 fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t nrows,
                  const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
-                 const float* __restrict__ gz) {
+                 const float* __restrict__ gz, int in_pitch) {
   extern __shared__ float2 smem[];
   constexpr int M = N / 2;
   using PL = Plan<M>;
@@ -225,7 +270,7 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
   const int p = threadIdx.x % P, g = threadIdx.x / P;
   const int64_t row = (int64_t)blockIdx.x * G + g;
   const bool ok = row < nrows;
-  const float2* src = in + row * (M + 1);
+  const float2* src = in + row * in_pitch;
   float2 v[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) {
@@ -258,62 +303,112 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
   for (int e = 0; e < E; ++e) dst[p + P * e] = make_float2(v[e].y * scale, v[e].x * scale);
 }
 
+// ---- TMA bulk copy + mbarrier (sm_90+/sm_100a) ------------------------------------------------------------
+// One elected thread arms the barrier with the byte count and issues cp.async.bulk; the copy engine writes
+// shared memory directly (no LSU data-pipe wavefronts, no registers) and completes the transaction count.
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+// global -> shared, bytes a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, uint64_t* bar) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(d), "l"(gsrc), "r"(bytes), "r"(b) : "memory");
+}
+
 // The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved
 // per cell as float4 (F_x, F_y, F_z, 0): the readout then needs one 16-byte gather per CIC corner
 // instead of three 4-byte ones (profiles/r01_B: the gather was request- and latency-bound).
 // A block owns GC rows; its three thread groups (GC*P threads each, whole warps) invert the rows of
 // component 0, 1, 2 concurrently, each with its own exchange buffer, park the real rows there, and
 // the block then writes its GC*N cells as fully coalesced float4.
+// The input rows (padded pitch: the GC rows of a component are one contiguous, 16-byte aligned run) arrive
+// by ONE TMA bulk copy per component into the exchange buffers: the Hermitian merge reads X[k] and X[M-k],
+// which as global loads fetched every element twice through L1 (profiles/r01_E: L1 data pipe 69 %, 60 % of
+// it global-load wavefronts).
 // g(w_z) of Eq. 5 is applied on load to component 2 (see fft_z_c2r_kernel).
 template <int N> __host__ __device__ constexpr int z3_rows() {
   constexpr int g = z_rows<N>() / 8;   // swept 2 / 4 / 8 at N = 512: 0.92 / 0.87 / 0.84 ms
-  return g < 1 ? 1 : g;
+  return g < 2 ? 2 : g;                // even, so a block's rows are a 16-byte multiple at any pitch
 }
 template <int N> __host__ __device__ constexpr int z3_threads() { return 3 * z3_rows<N>() * Plan<N / 2>::P; }
+template <int N> __host__ __device__ constexpr int z3_row_pitch() {
+  return row_pitch(N / 2) > padded_pitch(N) ? row_pitch(N / 2) : padded_pitch(N);
+}
 template <int N> __host__ __device__ constexpr size_t z3_smem_bytes() {
-  return sizeof(float2) * 3 * (size_t)z3_rows<N>() * row_pitch(N / 2);
+  return sizeof(float2) * 3 * (size_t)z3_rows<N>() * z3_row_pitch<N>() + 16;
 }
 
-template <int N>
+template <int N, bool TMA = true>
 __global__ void __launch_bounds__(z3_threads<N>())
 fft_z_c2r3_kernel(const float2* __restrict__ in0, const float2* __restrict__ in1,
                   const float2* __restrict__ in2, float4* __restrict__ out4, int64_t nrows,
                   const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
                   const float* __restrict__ gz) {
-  extern __shared__ float2 smem[];
-  constexpr int M = N / 2;
+  extern __shared__ __align__(128) float2 smem[];
+  constexpr int M = N / 2, PZ = padded_pitch(N);
   using PL = Plan<M>;
-  constexpr int E = PL::E, P = PL::P, GC = z3_rows<N>(), TG = GC * P, R = GC * row_pitch(M);
+  constexpr int E = PL::E, P = PL::P, GC = z3_rows<N>(), TG = GC * P, R = GC * z3_row_pitch<N>();
   static_assert(TG % 32 == 0 || TG * 3 <= 32, "component groups are whole warps");
+  static_assert((GC * PZ) % 2 == 0 && (R % 2) == 0, "bulk copies move 16-byte multiples to 16-byte aligned regions");
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + 3 * R);
   const int comp = threadIdx.x / TG, t = threadIdx.x % TG;
   const int p = t % P, g = t / P;
-  const int64_t row0 = (int64_t)blockIdx.x * GC, row = row0 + g;
-  const bool ok = row < nrows;
+  const int64_t row0 = (int64_t)blockIdx.x * GC, row = row0 + g;   // nrows = N^2 is a multiple of GC
   float2* region = smem + comp * R;
-  const float2* src = (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * (M + 1);
+  if (TMA) {
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      constexpr unsigned bytes = sizeof(float2) * GC * PZ;
+      mbar_expect_tx(bar, 3 * bytes);
+      bulk_load(smem, in0 + row0 * PZ, bytes, bar);
+      bulk_load(smem + R, in1 + row0 * PZ, bytes, bar);
+      bulk_load(smem + 2 * R, in2 + row0 * PZ, bytes, bar);
+    }
+    mbar_wait(bar, 0);
+  }
+  const float2* src = TMA ? region + g * PZ : (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * PZ;
   float2 v[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int k = p + P * e;
-    float2 z = make_float2(0.f, 0.f);
-    if (ok) {
-      float2 xk = src[k], xm = src[M - k];
-      if (comp == 2) {
-        const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
-        xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
-      }
-      if (k == 0) {
-        z = make_float2(xk.x + xm.x, xk.x - xm.x);
-      } else {
-        const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
-        const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
-        const float2 w = __ldg(twn + k);
-        const float2 b = cmul(d, make_float2(w.x, -w.y));
-        z = make_float2(a.x - b.y, a.y + b.x);
-      }
+    float2 xk = src[k], xm = src[M - k];
+    if (comp == 2) {
+      const float gk = __ldg(gz + k), gm = __ldg(gz + M - k);
+      xk.x *= gk; xk.y *= gk; xm.x *= gm; xm.y *= gm;
+    }
+    float2 z;
+    if (k == 0) {
+      z = make_float2(xk.x + xm.x, xk.x - xm.x);
+    } else {
+      const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
+      const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
+      const float2 w = __ldg(twn + k);
+      const float2 b = cmul(d, make_float2(w.x, -w.y));
+      z = make_float2(a.x - b.y, a.y + b.x);
     }
     v[e] = cswap(z);
   }
+  if (TMA) __syncthreads();                       // every input row is in registers: the regions become exchange buffers
   RowSmem sm{region + g * row_pitch(M)};
   fft_line<M>(v, p, sm, tw);
   if constexpr (PL::NST > 1) __syncthreads();   // exchange buffers free: park the real rows in them

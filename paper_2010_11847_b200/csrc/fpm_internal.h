@@ -43,18 +43,16 @@ struct ProfScope {
 
 // Opt a kernel in to more than 48 KB of dynamic shared memory, once per kernel and device (the attribute
 // is per device; calling cudaFuncSetAttribute before every launch showed up on the small configurations).
+cudaError_t ensure_dynamic_smem_impl(const void* kernel, size_t bytes);     // profiler.cpp
 template <class K>
 inline cudaError_t ensure_dynamic_smem(K kernel, size_t bytes) {
   if (bytes <= 48 * 1024) return cudaSuccess;
-  static bool done[64] = {};
-  int dev = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return e;
-  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
-  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-  if (e == cudaSuccess && dev >= 0 && dev < 64) done[dev] = true;
-  return e;
+  return ensure_dynamic_smem_impl(reinterpret_cast<const void*>(kernel), bytes);
 }
+
+// Tuning switches for A/B measurements (environment FPM_TUNE_<NAME>, read once); the defaults are the
+// measured winners and the product never depends on a switch being set.
+int tune(const char* name, int dflt);     // profiler.cpp
 
 // ---- FFT (fft.cu) ---------------------------------------------------------------------------
 struct FftTables {
@@ -92,9 +90,10 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
 // paint'ed density -> the three force meshes F[0..2] with the transfer function fused into the
 // transform passes (fft.cu); scale = 1.5 omega_m (or 1).  F4 != nullptr: the three components are
 // written interleaved per cell as float4 (x, y, z, unused) into F4[4 ng^3] instead of F[0..2].
+// batch > 1 (F4 only): every buffer holds `batch` meshes back to back and each pass covers them all
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof = nullptr);
+                            cudaStream_t s, Profiler* prof = nullptr, int batch = 1);
 
 // out = c2r[(scale / K^2) r2c[src]] with the multiplier fused into the x round trip (backward pass)
 cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
@@ -107,8 +106,9 @@ struct ParticleOrder {
   int np = 0;
   int paint_mode = FPM_PAINT_AUTO;
 };
+// batch > 1: [batch][3][n] positions, [batch][n] masses, [batch][ng^3] meshes in one launch (N2)
 cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
-                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s);
+                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s, int batch = 1);
 cudaError_t readout(const float* mesh, const float* pos, int64_t n, int ng, float* out,
                     const ParticleOrder& ord, cudaStream_t s);
 cudaError_t readout3(const float* fx, const float* fy, const float* fz, const float* pos, int64_t n,
@@ -138,7 +138,7 @@ cudaError_t drift(float* pos, const float* mom, int64_t n3, float fac, int ng, c
 // fy == fz == nullptr: fx is the interleaved float4 force mesh of fft_force_fused
 cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
                                float* mom, int64_t n, int ng, float kfac, float dfac,
-                               const ParticleOrder& ord, cudaStream_t s);
+                               const ParticleOrder& ord, cudaStream_t s, int batch = 1);
 
 // ---- transfer function and LPT element-wise kernels (green.cu) ---------------------------------
 cudaError_t apply_force_kernel(const KernelTables& kt, const float2* dk, float scale, float2* fkx,
@@ -193,4 +193,14 @@ struct fpm_ctx {
   bool sticky = false;
   std::string err;
   fpm::Profiler prof;
+  // whole-run CUDA graphs of fpm_nbody (api.cu): captured on an internal stream, replayed on `stream`
+  int graph_mode = FPM_GRAPH_AUTO;
+  cudaStream_t capture_stream = nullptr;
+  struct RunGraph {
+    float *pos, *mom, *traj;
+    std::vector<double> kf, dr;
+    cudaGraphExec_t exec;
+    long long launches;
+  };
+  std::vector<RunGraph> graphs;
 };

@@ -197,6 +197,10 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
   extern __shared__ __align__(16) float win_f[];
   __shared__ int red_i[3][kBrickThreads / 32];
   __shared__ float red_f[2][kBrickThreads / 32];
+  // blockIdx.y: simulation of a batch ([batch][3][n] particles, [batch][ng^3] meshes)
+  pos += (int64_t)blockIdx.y * 3 * n;
+  mesh += (int64_t)blockIdx.y * ng * ng * ng;
+  if (HAS_MASS) mass += (int64_t)blockIdx.y * n;
   const int mask = ng - 1;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   // sub-brick origin (lattice sites): np is a power of two, so the brick coordinates are bit fields
@@ -513,6 +517,10 @@ rkd_pipelined_kernel(const float* __restrict__ fx, const float* __restrict__ fy,
   constexpr int CPL = (NCP + 31) / 32;
   __shared__ __align__(16) float ring[STAGES][KB][6][kThreads];
   const float ng = (float)ngi, inv_ng = 1.f / ng;
+  // blockIdx.y: simulation of a batch (interleaved force mesh only: [batch][ng^3] float4)
+  pos += (int64_t)blockIdx.y * 3 * n;
+  mom += (int64_t)blockIdx.y * 3 * n;
+  if (F4) fx += (int64_t)blockIdx.y * 4 * ngi * ngi * ngi;
   const float* const mesh[3] = {fx, fy, fz};
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int qx0, qy0, qz0;
@@ -765,9 +773,10 @@ inline BrickMap brick_map(int np) { return BrickMap{np, np / BZ, np / BY, ilog2(
 }  // namespace
 
 cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t n, int ng,
-                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s) {
+                  float* mesh, bool zero_first, const ParticleOrder& ord, cudaStream_t s, int batch) {
+  const size_t g3 = (size_t)ng * ng * ng;
   if (zero_first) {
-    cudaError_t e = cudaMemsetAsync(mesh, 0, sizeof(float) * (size_t)ng * ng * ng, s);
+    cudaError_t e = cudaMemsetAsync(mesh, 0, sizeof(float) * g3 * batch, s);
     if (e != cudaSuccess) return e;
   }
   if (n == 0) return cudaSuccess;
@@ -778,11 +787,13 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
   if (mode == FPM_PAINT_AUTO) mode = can_brick ? FPM_PAINT_BRICK_FIXED : FPM_PAINT_DIRECT;
   if (mode != FPM_PAINT_DIRECT && !can_brick) mode = FPM_PAINT_DIRECT;
   if (mode == FPM_PAINT_DIRECT) {
-    paint_direct_kernel<<<blocks_for(n), kThreads, 0, s>>>(pos, mass, mass_const, n, ng, mesh);
+    for (int b = 0; b < batch; ++b)
+      paint_direct_kernel<<<blocks_for(n), kThreads, 0, s>>>(pos + (size_t)b * 3 * n, mass ? mass + (size_t)b * n : nullptr,
+                                                             mass_const, n, ng, mesh + b * g3);
     return cudaGetLastError();
   }
   const size_t smem = sizeof(float) * (size_t)kWinCells;
-  const unsigned grid = (unsigned)(n / (kBrick / (res * res * res)));
+  const dim3 grid((unsigned)(n / (kBrick / (res * res * res))), (unsigned)batch);
   const BrickMap bm = brick_map(ord.np);
   auto go = [&](auto kern) -> cudaError_t {
     cudaError_t e = ensure_dynamic_smem(kern, smem);
@@ -828,12 +839,13 @@ cudaError_t readout3(const float* fx, const float* fy, const float* fz, const fl
 
 cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz, float* pos,
                                float* mom, int64_t n, int ng, float kfac, float dfac,
-                               const ParticleOrder& ord, cudaStream_t s) {
+                               const ParticleOrder& ord, cudaStream_t s, int batch) {
   if (n == 0) return cudaSuccess;
   const bool f4 = (fy == nullptr);   // interleaved force mesh
+  if (batch > 1 && !f4) return cudaErrorInvalidValue;      // batches run the fused path only
   const bool aligned = ((reinterpret_cast<uintptr_t>(pos) | reinterpret_cast<uintptr_t>(mom)) & 15) == 0;
   if (brick_ok(n, ord.np) && aligned) {
-    const unsigned grid = (unsigned)(2 * (n / kBrick));
+    const dim3 grid((unsigned)(2 * (n / kBrick)), (unsigned)batch);
     const BrickMap bm = brick_map(ord.np);
     if (f4)
       rkd_pipelined_kernel<3, 1, 4, true><<<grid, kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, bm, kfac, dfac);
@@ -841,10 +853,13 @@ cudaError_t readout_kick_drift(const float* fx, const float* fy, const float* fz
       rkd_pipelined_kernel<3, 1, 4, false><<<grid, kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, bm, kfac, dfac);
     return cudaGetLastError();
   }
-  if (f4)
-    readout_kick_drift_kernel<true><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, kfac, dfac);
-  else
+  if (f4) {
+    for (int b = 0; b < batch; ++b)
+      readout_kick_drift_kernel<true><<<blocks_for(n), kThreads, 0, s>>>(
+          fx + (size_t)b * 4 * ng * ng * ng, fy, fz, pos + (size_t)b * 3 * n, mom + (size_t)b * 3 * n, n, ng, kfac, dfac);
+  } else {
     readout_kick_drift_kernel<false><<<blocks_for(n), kThreads, 0, s>>>(fx, fy, fz, pos, mom, n, ng, kfac, dfac);
+  }
   return cudaGetLastError();
 }
 

@@ -1,8 +1,42 @@
 // profiler.cpp -- per-kernel CUDA-event timing on the context's stream (used by bench.py for the
 // live roofline numbers) and the launch counter behind fpm_launch_count().
+#include <cstdlib>
+#include <map>
+#include <string>
+#include <mutex>
+#include <utility>
+
 #include "fpm_internal.h"
 
 namespace fpm {
+
+int tune(const char* name, int dflt) {
+  static std::mutex mu;
+  static std::map<std::string, int> cache;
+  std::lock_guard<std::mutex> lock(mu);
+  auto it = cache.find(name);
+  if (it != cache.end()) return it->second;
+  const std::string key = std::string("FPM_TUNE_") + name;
+  const char* v = std::getenv(key.c_str());
+  const int val = v ? std::atoi(v) : dflt;
+  cache[name] = val;
+  return val;
+}
+
+// (kernel, device) pairs whose MaxDynamicSharedMemorySize attribute is already raised to >= bytes
+cudaError_t ensure_dynamic_smem_impl(const void* kernel, size_t bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<const void*, int>, size_t> done;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& have = done[std::make_pair(kernel, dev)];
+  if (have >= bytes) return cudaSuccess;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) have = bytes;
+  return e;
+}
 
 const char* kernel_name(int kid) {
   static const char* names[K_COUNT] = {

@@ -37,18 +37,22 @@ def test_argument_validation_needs_no_gpu():
         _fields_ = [("ng", ctypes.c_int32), ("np", ctypes.c_int32), ("omega_m", ctypes.c_double),
                     ("box", ctypes.c_double), ("kernel_mode", ctypes.c_int32),
                     ("factor_mode", ctypes.c_int32), ("force_path", ctypes.c_int32),
-                    ("paint_mode", ctypes.c_int32)]
+                    ("paint_mode", ctypes.c_int32), ("batch", ctypes.c_int32)]
 
     lib.fpm_workspace_bytes.restype = ctypes.c_size_t
     good = Cfg(512, 512, 0.3075, 1000.0, 0, 0, 0, 0)
-    nk = 512 * 512 * 257
-    assert lib.fpm_workspace_bytes(ctypes.byref(good)) == 4 * 512 ** 3 * 4 + 4 * nk * 8
+    nk = 512 * 512 * 272          # half-complex scratch rows are padded to 16 elements (128 bytes)
+    assert lib.fpm_workspace_bytes(ctypes.byref(good)) == 4 * 512 ** 3 * 4 + 4 * nk * 8 + 4 * 37 * 256
     for bad in (Cfg(500, 500, 0.3, 0, 0, 0, 0, 0), Cfg(64, 128, 0.3, 0, 0, 0, 0, 0),
                 Cfg(2048, 2048, 0.3, 0, 0, 0, 0, 0), Cfg(64, 64, -1.0, 0, 0, 0, 0, 0),
-                Cfg(64, 64, 0.3, 0, 7, 0, 0, 0), Cfg(64, 64, 0.3, 0, 0, 0, 0, 9), Cfg(64, 64, 0.3, 0, 0, 0, 5, 0)):
+                Cfg(64, 64, 0.3, 0, 7, 0, 0, 0), Cfg(64, 64, 0.3, 0, 0, 0, 0, 9), Cfg(64, 64, 0.3, 0, 0, 0, 5, 0),
+                Cfg(64, 64, 0.3, 0, 0, 0, 0, 0, -1), Cfg(64, 64, 0.3, 0, 0, 0, 0, 0, 4),      # a batch needs the fused path
+                Cfg(64, 16, 0.3, 0, 0, 0, 1, 0, 4), Cfg(1024, 1024, 0.3, 0, 0, 0, 1, 0, 64)):
         assert lib.fpm_workspace_bytes(ctypes.byref(bad)) == 0
         h = ctypes.c_void_p()
         assert lib.fpm_create(ctypes.byref(bad), None, ctypes.byref(h)) == -1
+    batched = Cfg(128, 128, 0.3075, 200.0, 0, 0, 1, 0, 16)
+    assert lib.fpm_workspace_bytes(ctypes.byref(batched)) == 16 * (4 * 128 ** 3 * 4 + 4 * 128 * 128 * 80 * 8) + 4 * 37 * 256
     assert lib.fpm_destroy(None) == -1
     assert lib.fpm_paint(None, None, None, ctypes.c_int64(0), None) == -1
     # calls added for the backward pass and N1 validate the same way

@@ -185,4 +185,4 @@ def test_paint_with_badly_conditioned_and_non_finite_masses(fpm, oracle):
     finite_ref = oracle.paint(pos.astype(np.float64), ng, mass=np.where(np.isfinite(bad), mass, 0.0).astype(np.float64))
     ok = np.isfinite(got)
     assert ok.sum() >= got.size - 16
-    assert np.max(np.abs(got[ok] - finite_ref[ok])) < 1e-3
+    assert np.max(np.abs(got[ok] - finite_ref[ok]) - 2e-7 * np.abs(finite_ref[ok])) < 1e-3

@@ -163,3 +163,21 @@ def test_power_spectrum_of_a_single_mode_and_of_the_linear_field(oracle):
     # cross spectrum with itself is the auto spectrum (Eq. 11: r_c = 1)
     _, pab, _ = oracle.power(1.0 + d, box, mesh_b=1.0 + d)
     assert np.allclose(pab, pk, rtol=1e-12)
+
+
+def test_batch_of_runs_equals_the_single_runs_and_its_members_are_independent(oracle):
+    """N2 pin: the batch is defined as B independent runs, so member b must be bit-for-bit the single run of
+    its inputs, and changing one member's input must leave every other member's output untouched."""
+    n, ng = 8, 8
+    stages = [0.1, 0.4, 0.7, 1.0]
+    states = [oracle.lpt_init(0.5 * fi.linear_field(n, 60.0, seed=s).astype(np.float64), ng, OM, 0.1, 2) for s in (1, 2, 3)]
+    pos = np.stack([p for p, _ in states])
+    mom = np.stack([m for _, m in states])
+    bp, bm = oracle.nbody_batch(pos, mom, ng, n, OM, stages)
+    for b in range(3):
+        sp, sm = oracle.nbody(pos[b], mom[b], ng, n, OM, stages)
+        assert np.array_equal(bp[b], sp) and np.array_equal(bm[b], sm)
+    pos2 = pos.copy()
+    pos2[1] = np.mod(pos2[1] + 0.37, ng)
+    cp, cm = oracle.nbody_batch(pos2, mom, ng, n, OM, stages)
+    assert np.array_equal(cp[0], bp[0]) and np.array_equal(cp[2], bp[2]) and not np.array_equal(cp[1], bp[1])
