@@ -285,6 +285,23 @@ int fpm_recon_loss_grad(fpm_ctx* ctx, const float* s, const float* data, double 
 int fpm_adam_step(fpm_ctx* ctx, float* x, const float* grad, float* m, float* v, int64_t n, double lr,
                   double beta1, double beta2, double eps, int t);
 
+/* ---- multi-grid pyramid (Eq. 6-9, Alg. 2-3) ------------
+ * The paper's two-level force scheme, built for its distributed FFT; on one GPU it is strictly more work than
+ * the single-mesh force, so it is offered for accuracy studies, not used by fpm_nbody.
+ * BSpline(6) is read as the two-scale mask of the order-6 cardinal B-spline, [1, 6, 15, 20, 15, 6, 1]/64 per
+ * axis (R14).  All three calls need the workspace; levels >= 0 with ng >> levels >= 8. */
+
+/* Alg. 2 REDUCE: `levels` consecutive periodic stride-2 convolutions with the mask.  in [ng^3] -> out
+ * [(ng >> levels)^3]; out must not alias in. */
+int fpm_reduce(fpm_ctx* ctx, const float* in, int levels, float* out);
+/* Alg. 2 EXPAND: `levels` consecutive transposed stride-2 convolutions with 8 x the mask.
+ * in [(ng >> levels)^3] -> out [ng^3]. */
+int fpm_expand(fpm_ctx* ctx, const float* in, int levels, float* out);
+/* Alg. 3 Force: force [3][n] at pos from F = EXPAND(2^levels ForceGrids(REDUCE(rho))) + F_S - EXPAND(REDUCE(F_S)),
+ * F_S = ForceGrids(rho) the single-mesh force meshes, rho = paint(pos); already x 1.5 omega_m like fpm_force.
+ * (The factor 2^levels converts the coarse mesh's force per coarse cell spacing into fine-cell units.) */
+int fpm_force_pyramid(fpm_ctx* ctx, const float* pos, int64_t n, int levels, float* force);
+
 /* ---- measurement hooks -------------------------------------------------------------------- */
 /* Per-kernel CUDA-event timing on the context's stream (off by default).  fpm_profile_read
  * synchronises the recorded events; kernel_id runs over 0 .. until FPM_EINVAL is returned.

@@ -82,6 +82,9 @@ def _load():
                                       ctypes.POINTER(dbl)]),
         "fpm_adam_step": (i32, [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, i32]),
         "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
+        "fpm_reduce": (i32, [vp, vp, i32, vp]),
+        "fpm_expand": (i32, [vp, vp, i32, vp]),
+        "fpm_force_pyramid": (i32, [vp, vp, i64, i32, vp]),
         "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
     }
     for name, (res, args) in sig.items():
@@ -394,6 +397,25 @@ class FPM:
                                           order, _dev(grad_pos, numel=n3, what="grad_pos"),
                                           _dev(grad_mom, numel=n3, what="grad_mom"), _dev(out)))
         return out
+
+    # ---- multi-grid pyramid (Alg. 2-3) -----------------------------------
+    def reduce(self, mesh, levels=2):
+        nc = self.ng >> levels
+        out = self._empty(nc, nc, nc)
+        self._check(_lib.fpm_reduce(self._h, _dev(mesh, numel=self._n_g, what="mesh"), int(levels), _dev(out)))
+        return out
+
+    def expand(self, mesh, levels=2):
+        nc = self.ng >> levels
+        out = self._empty(self.ng, self.ng, self.ng)
+        self._check(_lib.fpm_expand(self._h, _dev(mesh, numel=nc ** 3, what="coarse mesh"), int(levels), _dev(out)))
+        return out
+
+    def force_pyramid(self, pos, levels=2):
+        n = _particles(pos)
+        f = self._empty(3, n)
+        self._check(_lib.fpm_force_pyramid(self._h, _dev(pos), n, int(levels), _dev(f)))
+        return f
 
     # ---- MAP reconstruction (Eq. 12, Listing 7.1) -------------------
     def recon_loss_grad(self, s, data, sigma, inv_power, stages, lpt_order=2, scratch=None):

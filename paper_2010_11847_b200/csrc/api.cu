@@ -138,7 +138,8 @@ int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, 
     FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s, batch)); }
   if (ctx->cfg.force_path == FPM_FORCE_FUSED) {
     FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F,
-                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr, batch));
+                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr, batch,
+                                  &ctx->maps));
     return FPM_OK;
   }
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
@@ -193,7 +194,8 @@ int force_vjp(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, con
       FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.F[d], true, ord, s));
     }
     { ProfScope sc2(pr, K_GREEN); FPM_CUDA(ctx, stencil_divergence(w.F[0], w.F[1], w.F[2], ng, w.rho, s)); }
-    FPM_CUDA(ctx, fft_poisson(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.F[0], (float)(-coef * sc), s, pr));
+    FPM_CUDA(ctx, fft_poisson(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.F[0], (float)(-coef * sc), s, pr,
+                              ctx->maps.ok ? &ctx->maps.x[0] : nullptr));
   } else {
     for (int d = 0; d < 3; ++d) {
       { ProfScope sc2(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, v + d * n, 0.f, n, ng, w.rho, true, ord, s)); }
@@ -272,6 +274,8 @@ int fpm_destroy(fpm_ctx* ctx) {
   if (ctx->d_acc) cudaFree(ctx->d_acc);
   fft_tables_destroy(&ctx->fft_g);
   fft_tables_destroy(&ctx->fft_p);
+  fft_tables_destroy(&ctx->fft_c);
+  kernel_tables_destroy(&ctx->kt_c);
   kernel_tables_destroy(&ctx->kt_g);
   kernel_tables_destroy(&ctx->kt_p);
   delete ctx;
@@ -288,6 +292,9 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
   drop_graphs(ctx);
   ctx->ws = ws;
   ctx->ws_bytes = bytes;
+  const Workspace w = carve(ctx);
+  float2* const bufs[4] = {w.dk, w.fk[0], w.fk[1], w.fk[2]};
+  FPM_CUDA(ctx, fft_make_tile_maps(ctx->cfg.ng, batch_of(ctx->cfg), bufs, &ctx->maps));
   return FPM_OK;
 }
 
@@ -813,6 +820,133 @@ int fpm_adam_step(fpm_ctx* ctx, float* x, const float* grad, float* m, float* v,
   const double c1 = 1.0 - std::pow(beta1, t), c2 = 1.0 - std::pow(beta2, t);
   ctx->prof.launches += 1;
   FPM_CUDA(ctx, adam_update(x, grad, m, v, n, lr, beta1, beta2, eps, 1.0 / c1, 1.0 / c2, ctx->stream));
+  return FPM_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+inline int64_t cube(int64_t n) { return n * n * n; }
+
+// REDUCE in (n^3) by `levels` levels into out; scratch: n^3 floats (3/4 + 1/8 of each level's mesh)
+int pyr_reduce(fpm_ctx* ctx, const float* in, int n, int levels, float* scratch, float* out) {
+  if (levels == 0) {
+    FPM_CUDA(ctx, cudaMemcpyAsync(out, in, sizeof(float) * cube(n), cudaMemcpyDeviceToDevice, ctx->stream));
+    return FPM_OK;
+  }
+  const float* cur = in;
+  for (int l = 0; l < levels; ++l) {
+    float* tmp = scratch;
+    float* dst = (l == levels - 1) ? out : scratch + 3 * cube(n) / 4;
+    ctx->prof.launches += 3;
+    FPM_CUDA(ctx, pyramid_reduce_level(cur, n, tmp, dst, ctx->stream));
+    scratch += 3 * cube(n) / 4 + cube(n / 2);
+    cur = dst;
+    n /= 2;
+  }
+  return FPM_OK;
+}
+
+// EXPAND in (m^3) by `levels` levels into out ((m << levels)^3); scratch: (m << levels)^3 floats
+int pyr_expand(fpm_ctx* ctx, const float* in, int m, int levels, float* scratch, float* out) {
+  if (levels == 0) {
+    FPM_CUDA(ctx, cudaMemcpyAsync(out, in, sizeof(float) * cube(m), cudaMemcpyDeviceToDevice, ctx->stream));
+    return FPM_OK;
+  }
+  const float* cur = in;
+  for (int l = 0; l < levels; ++l) {
+    float* tmp = scratch;
+    float* dst = (l == levels - 1) ? out : scratch + 6 * cube(m);
+    ctx->prof.launches += 3;
+    FPM_CUDA(ctx, pyramid_expand_level(cur, m, tmp, dst, ctx->stream));
+    scratch += 6 * cube(m) + 8 * cube(m);
+    cur = dst;
+    m *= 2;
+  }
+  return FPM_OK;
+}
+
+bool pyramid_levels_ok(const fpm_ctx* ctx, int levels) {
+  return levels >= 0 && levels < 8 && (ctx->cfg.ng >> levels) >= 8;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fpm_reduce(fpm_ctx* ctx, const float* in, int levels, float* out) {
+  FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_reduce");
+  FPM_REQUIRE(ctx, in && out && in != out, "fpm_reduce: bad arguments");
+  FPM_REQUIRE(ctx, pyramid_levels_ok(ctx, levels), "fpm_reduce: levels out of range (ng >> levels >= 8)");
+  FPM_NEED_WS(ctx);
+  return pyr_reduce(ctx, in, ctx->cfg.ng, levels, reinterpret_cast<float*>(carve(ctx).dk), out);
+}
+
+int fpm_expand(fpm_ctx* ctx, const float* in, int levels, float* out) {
+  FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_expand");
+  FPM_REQUIRE(ctx, in && out && in != out, "fpm_expand: bad arguments");
+  FPM_REQUIRE(ctx, pyramid_levels_ok(ctx, levels), "fpm_expand: levels out of range (ng >> levels >= 8)");
+  FPM_NEED_WS(ctx);
+  return pyr_expand(ctx, in, ctx->cfg.ng >> levels, levels, reinterpret_cast<float*>(carve(ctx).dk), out);
+}
+
+int fpm_force_pyramid(fpm_ctx* ctx, const float* pos, int64_t n, int levels, float* force) {
+  FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_force_pyramid");
+  FPM_REQUIRE(ctx, n >= 0 && ((pos && force) || n == 0), "fpm_force_pyramid: bad arguments");
+  FPM_REQUIRE(ctx, pyramid_levels_ok(ctx, levels), "fpm_force_pyramid: levels out of range (ng >> levels >= 8)");
+  FPM_NEED_WS(ctx);
+  const Workspace w = carve(ctx);
+  cudaStream_t s = ctx->stream;
+  Profiler* pr = &ctx->prof;
+  const int ng = ctx->cfg.ng, nc = ng >> levels;
+  const float scale = (float)(1.5 * ctx->cfg.omega_m);
+  if (ctx->coarse_n != nc) {                      // plans of the coarse mesh, kept for the next call
+    fft_tables_destroy(&ctx->fft_c);
+    kernel_tables_destroy(&ctx->kt_c);
+    ctx->coarse_n = 0;
+    FPM_CUDA(ctx, fft_tables_create(nc, &ctx->fft_c));
+    FPM_CUDA(ctx, kernel_tables_create(nc, ctx->cfg.kernel_mode, &ctx->kt_c));
+    ctx->coarse_n = nc;
+  }
+  // F_S <= ForceGrids(H, local): the single-mesh force meshes, op by op (Alg. 3 ForceGrids)
+  { ProfScope sc(pr, K_PAINT); FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s)); }
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
+  { ProfScope sc(pr, K_GREEN); FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, w.dk, scale, w.fk[0], w.fk[1], w.fk[2], s)); }
+  for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.fk[d], w.F[d], s, pr));
+  // the four half-complex regions are free now; each holds two real meshes
+  const int64_t g3 = cube(ng), c3 = cube(nc);
+  float* scratch = reinterpret_cast<float*>(w.dk);            // pyr_reduce / pyr_expand scratch (g3 floats)
+  float* up = reinterpret_cast<float*>(w.fk[0]);              // EXPAND(F_L)
+  float* lowup = up + g3;                                     // EXPAND(REDUCE(F_S))
+  float* coarse = reinterpret_cast<float*>(w.fk[1]);          // D | F_L[3] | low
+  float* D = coarse;
+  float* FL[3] = {coarse + c3, coarse + 2 * c3, coarse + 3 * c3};
+  float* low = coarse + 4 * c3;
+  float2* ck = reinterpret_cast<float2*>(w.fk[2]);            // coarse spectra: dk | fk[3]
+  const int64_t ckn = (int64_t)nc * nc * (nc / 2 + 1);
+  // D <= REDUCE(H);  F_L <= ForceGrids(D, distributed), in fine-cell units
+  int rc = pyr_reduce(ctx, w.rho, ng, levels, scratch, D);
+  if (rc != FPM_OK) return rc;
+  FPM_CUDA(ctx, fft_r2c(ctx->fft_c, D, ck, s, pr));
+  { ProfScope sc(pr, K_GREEN);
+    FPM_CUDA(ctx, apply_force_kernel(ctx->kt_c, ck, scale * (float)(1 << levels), ck + ckn, ck + 2 * ckn, ck + 3 * ckn, s)); }
+  for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_c, ck + (d + 1) * ckn, FL[d], s, pr));
+  for (int d = 0; d < 3; ++d) {
+    rc = pyr_expand(ctx, FL[d], nc, levels, scratch, up);          // F_iL <= EXPAND(F_iL)
+    if (rc != FPM_OK) return rc;
+    rc = pyr_reduce(ctx, w.F[d], ng, levels, scratch, low);        // F_il <= REDUCE(F_iS)
+    if (rc != FPM_OK) return rc;
+    rc = pyr_expand(ctx, low, nc, levels, scratch, lowup);         // F_il <= EXPAND(F_il)
+    if (rc != FPM_OK) return rc;
+    ctx->prof.launches += 1;
+    FPM_CUDA(ctx, pyramid_combine(w.F[d], up, lowup, g3, s));      // F_i <= F_iL + (F_iS - F_il)
+  }
+  ProfScope sc(pr, K_READOUT);
+  FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ng, force, order_of(ctx, n), s));
   return FPM_OK;
 }
 

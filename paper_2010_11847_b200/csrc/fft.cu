@@ -133,11 +133,28 @@ cudaError_t c2r_impl(const FftTables& t, float2* cplx, float* real, cudaStream_t
 // internal, with the padded row pitch PZ = padded_pitch(N) (128-byte aligned rows and 16-column tiles).
 template <int N>
 cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, const float2* in, float2* out_a,
-                                float2* out_bx, float scale, bool poisson, cudaStream_t s, int batch = 1) {
+                                float2* out_bx, float scale, bool poisson, cudaStream_t s, int batch = 1,
+                                const CUtensorMap* m_in = nullptr, const CUtensorMap* m_a = nullptr,
+                                const CUtensorMap* m_bx = nullptr) {
   constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N), TX = xf_tile<N>();
   const dim3 grid((nzh + TX - 1) / TX, N, batch);
   const unsigned threads = TX * Plan<N, xf_variant<N>()>::P;
   cudaError_t e;
+  if (m_in && m_a && (poisson || m_bx) && tune("TMA", 1)) {     // TMA tile movers
+    const size_t smem = xf_tma_smem_bytes<N>();
+    if (poisson) {
+      auto kern = fft_x_force_tma_kernel<N, true>;
+      e = set_smem(kern, smem);
+      if (e != cudaSuccess) return e;
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_a, t.stage_x, kt.lap, kt.grad, scale);
+    } else {
+      auto kern = fft_x_force_tma_kernel<N, false>;
+      e = set_smem(kern, smem);
+      if (e != cudaSuccess) return e;
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
+    }
+    return cudaGetLastError();
+  }
   auto go = [&](auto kern) -> cudaError_t {
     e = set_smem(kern, xf_smem_bytes<N>());
     if (e != cudaSuccess) return e;
@@ -166,8 +183,9 @@ cudaError_t launch_z_r2c_padded(const FftTables& t, const float* real, float2* c
 template <int N>
 cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                              float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                             cudaStream_t s, Profiler* prof, int batch) {
+                             cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps) {
   constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N);
+  const bool tma = maps && maps->ok;
   // a batch of meshes back to back: its z rows and its x slabs are just more rows / slabs; only the x
   // round trip, whose lines stride across a whole mesh, takes the mesh index as a grid dimension
   if (batch < 1 || (batch > 1 && !F4) || (int64_t)N * batch > 65535) return cudaErrorInvalidValue;
@@ -186,14 +204,24 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
-    e = launch_x_round_trip<N>(t, kt, dk, wa, wb, scale, false, s, batch);
+    e = launch_x_round_trip<N>(t, kt, dk, wa, wb, scale, false, s, batch, tma ? &maps->x[0] : nullptr,
+                               tma ? &maps->x[1] : nullptr, tma ? &maps->x[2] : nullptr);
     if (e != cudaSuccess) return e;
   }
   {
     ProfScope sc(prof, K_FFT_Y_INV3);
     using YPL = Plan<N, yi_variant<N>()>;
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    if (tune("YPAIR", 1)) {
+    if (tma && tune("TMA", 1)) {
+      constexpr int TY = yi_tile<N>();
+      const size_t ysmem = sizeof(float2) * N * TY + 16;
+      auto kern = fft_y_inv3_tma_kernel<N>;
+      e = set_smem(kern, ysmem);
+      if (e != cudaSuccess) return e;
+      dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
+      kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
+                                                yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+    } else if (tune("YPAIR", 1)) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
       auto kern = fft_y_inv3_pair_kernel<N>;
@@ -240,7 +268,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
 // with the multiplier fused into the x round trip; work: one half-complex scratch buffer (padded pitch).
 template <int N>
 cudaError_t poisson_impl(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
-                         float scale, cudaStream_t s, Profiler* prof) {
+                         float scale, cudaStream_t s, Profiler* prof, const CUtensorMap* work_map_x) {
   constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N);
   cudaError_t e;
   {
@@ -255,7 +283,7 @@ cudaError_t poisson_impl(const FftTables& t, const KernelTables& kt, const float
   }
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
-    e = launch_x_round_trip<N>(t, kt, work, work, nullptr, scale, true, s);
+    e = launch_x_round_trip<N>(t, kt, work, work, nullptr, scale, true, s, 1, work_map_x, work_map_x, nullptr);
     if (e != cudaSuccess) return e;
   }
   {
@@ -267,6 +295,66 @@ cudaError_t poisson_impl(const FftTables& t, const KernelTables& kt, const float
 }
 
 }  // namespace
+
+namespace {
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// the driver entry point, without linking libcuda
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    cudaGetLastError();
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+template <int N>
+cudaError_t make_maps_impl(int batch, float2* const bufs[4], TileMaps* out) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  out->ok = false;
+  if (!enc) return cudaSuccess;
+  constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N), BOXR = tma_box_rows<N>();
+  // a mesh as a 3-D tensor of 8-byte elements: (kz < nzh, pitch PZ) x (y < N) x (x slab < N batch)
+  const cuuint64_t dims[3] = {(cuuint64_t)nzh, (cuuint64_t)N, (cuuint64_t)N * batch};
+  const cuuint64_t strides[2] = {sizeof(float2) * (cuuint64_t)PZ, sizeof(float2) * (cuuint64_t)PZ * N};
+  const cuuint32_t ones[3] = {1, 1, 1};
+  const cuuint32_t box_y[3] = {(cuuint32_t)yi_tile<N>(), (cuuint32_t)BOXR, 1};
+  const cuuint32_t box_x[3] = {(cuuint32_t)xf_tile<N>(), 1, (cuuint32_t)BOXR};
+  for (int i = 0; i < 4; ++i) {
+    if (enc(&out->y[i], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, bufs[i], dims, strides, box_y, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaSuccess;
+    if (enc(&out->x[i], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, bufs[i], dims, strides, box_x, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaSuccess;
+  }
+  out->ok = true;
+  return cudaSuccess;
+}
+}  // namespace
+
+cudaError_t fft_make_tile_maps(int n, int batch, float2* const bufs[4], TileMaps* out) {
+  switch (n) {
+    case 8: return make_maps_impl<8>(batch, bufs, out);
+    case 16: return make_maps_impl<16>(batch, bufs, out);
+    case 32: return make_maps_impl<32>(batch, bufs, out);
+    case 64: return make_maps_impl<64>(batch, bufs, out);
+    case 128: return make_maps_impl<128>(batch, bufs, out);
+    case 256: return make_maps_impl<256>(batch, bufs, out);
+    case 512: return make_maps_impl<512>(batch, bufs, out);
+    case 1024: return make_maps_impl<1024>(batch, bufs, out);
+    default: return cudaErrorInvalidValue;
+  }
+}
 
 bool fft_size_supported(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
 
@@ -323,16 +411,16 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
 }
 
 cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
-                        float scale, cudaStream_t s, Profiler* prof) {
+                        float scale, cudaStream_t s, Profiler* prof, const CUtensorMap* work_map_x) {
   if (kt.n != t.n) return cudaErrorInvalidValue;
-  FPM_FFT_DISPATCH(poisson_impl, t, kt, src, work, out, scale, s, prof)
+  FPM_FFT_DISPATCH(poisson_impl, t, kt, src, work, out, scale, s, prof, work_map_x)
 }
 
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof, int batch) {
+                            cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps) {
   if (kt.n != t.n) return cudaErrorInvalidValue;
-  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof, batch)
+  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof, batch, maps)
 }
 
 }  // namespace fpm

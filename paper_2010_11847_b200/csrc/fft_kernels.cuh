@@ -5,6 +5,8 @@
 //                      PAPER.md:49-59, rides on the x pass)
 //   fft_z_c2r_kernel : contiguous axis, half-complex -> real, merge + N/2-point inverse FFT
 #pragma once
+#include <cuda.h>
+
 #include "fft.cuh"
 
 namespace fpm {
@@ -332,6 +334,163 @@ __device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsi
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(d), "l"(gsrc), "r"(bytes), "r"(b) : "memory");
+}
+
+// 3-D tiled tensor copies (cp.async.bulk.tensor): one instruction moves a box of up to 256 lines x 128 bytes
+// between a half-complex mesh (dims kz, y, x-slab; padded pitch) and a dense shared-memory tile.  Columns
+// beyond n/2 + 1 are out of bounds for the tensor map: zero-filled on load, dropped on store.
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint64_t* bar) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(d), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(b) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, int c0, int c1, int c2, const void* smem_src) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_src);
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(reinterpret_cast<uint64_t>(map)), "r"(sa), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes to shared memory -> visible to the async proxy (before a TMA store reads them)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int N> __host__ __device__ constexpr int tma_box_rows() { return N < 256 ? N : 256; }
+
+// The three inverse y passes (see fft_y_inv3_pair_kernel) with the tiles moved by TMA: the whole 16-column
+// tile (N lines x 128 bytes) lands in shared memory with N / 256 tensor copies issued by one thread, the
+// transform runs register-resident out of it, the exchange reuses the same tile, and the result leaves by
+// TMA stores.  No global load or store goes through the LSU data pipe, which bounded the ld.global version
+// (profiles/r01_E: L1 data-pipe 85 %, 56 % of it global accesses).
+template <int N>
+__global__ void __launch_bounds__(yi_threads<N>())
+fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_constant__ CUtensorMap m_a,
+                      const __grid_constant__ CUtensorMap m_y, const __grid_constant__ CUtensorMap m_z,
+                      const float2* __restrict__ tw, const float* __restrict__ grad) {
+  extern __shared__ __align__(128) float2 smem[];
+  using PL = Plan<N, yi_variant<N>()>;
+  constexpr int T = yi_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + N * T);
+  const int c2 = threadIdx.x % (T / 2), p = threadIdx.x / (T / 2);
+  const int variant = blockIdx.x % 3, col0 = (blockIdx.x / 3) * T, slab = blockIdx.y;
+  const CUtensorMap* in = variant == 0 ? &m_bx : &m_a;
+  const CUtensorMap* out = variant == 0 ? &m_bx : (variant == 1 ? &m_y : &m_z);
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(bar, (unsigned)(sizeof(float2) * N * T));
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_load_3d(smem + b * BOXR * T, in, col0, b * BOXR, slab, bar);
+  }
+  mbar_wait(bar, 0);
+  float4* tile4 = reinterpret_cast<float4*>(smem);
+  cpair v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    float4 q = tile4[i * (T / 2) + c2];
+    if (variant == 1) { const float g = __ldg(grad + i); q.x *= g; q.y *= g; q.z *= g; q.w *= g; }
+    v[e] = cpair{make_float2(q.y, q.x), make_float2(q.w, q.z)};     // (im, re)-swapped: inverse transform
+  }
+  if constexpr (PL::NST > 1) __syncthreads();       // the landed tile is in registers: it becomes the exchange buffer
+  ColSmem2<T> sm{tile4, c2};
+  fft_line_plan<PL>(v, p, sm, tw);
+  if constexpr (PL::NST > 1) __syncthreads();       // last exchange read: the tile becomes the output stage
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    tile4[(p + P * e) * (T / 2) + c2] = make_float4(v[e].a.y, v[e].a.x, v[e].b.y, v[e].b.x);
+  fence_proxy_async();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_store_3d(out, col0, b * BOXR, slab, smem + b * BOXR * T);
+    tma_store_commit();
+    tma_store_wait_read();
+  }
+}
+
+// The fused x round trip (see fft_x_force_kernel) with TMA tiles: input tile -> stage buffer; A leaves from the
+// stage buffer and Bx from the park buffer while the next transform runs, so no store is waited for before
+// the end.  Shared memory = [exchange | park | stage] (3 N T complex) + the barrier.
+template <int N> __host__ __device__ constexpr size_t xf_tma_smem_bytes() {
+  return sizeof(float2) * 3 * (size_t)N * xf_tile<N>() + 16;
+}
+
+template <int N, bool POISSON = false>
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
+fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
+                       const __grid_constant__ CUtensorMap m_bx, const float2* __restrict__ tw,
+                       const float* __restrict__ lap, const float* __restrict__ grad, float scale) {
+  extern __shared__ __align__(128) float2 smem[];
+  using PL = Plan<N, xf_variant<N>()>;
+  constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
+  float2* xch = smem;
+  float2* park_tile = smem + N * T;
+  float2* stage = smem + 2 * N * T;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + 3 * N * T);
+  const int c = threadIdx.x % T, p = threadIdx.x / T;
+  const int y = blockIdx.y, col0 = blockIdx.x * T, kz = col0 + c, x0 = blockIdx.z * N;
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(bar, (unsigned)(sizeof(float2) * N * T));
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_load_3d(stage + b * BOXR * T, &m_in, col0, y, x0 + b * BOXR, bar);
+  }
+  mbar_wait(bar, 0);
+  float2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) v[e] = stage[(p + P * e) * T + c];
+  ColSmem<T> sm{xch, c};
+  fft_line_plan<PL>(v, p, sm, tw);
+  const float lyz = __ldg(lap + y) + __ldg(lap + (kz <= N / 2 ? kz : 0));
+  float2* park = park_tile + threadIdx.x;              // element e of this thread at park[e * T * P]
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = p + P * e;
+    const float k2 = __ldg(lap + i) + lyz;
+    const float f = ((y | kz | i) == 0) ? 0.f : scale / k2;
+    if constexpr (POISSON) {
+      v[e] = make_float2(v[e].y * f, v[e].x * f);        // f v, (im, re)-swapped
+    } else {
+      v[e] = make_float2(v[e].x * f, -v[e].y * f);       // i f v, (im, re)-swapped
+      park[e * (T * P)] = v[e];
+    }
+  }
+  if constexpr (PL::NST > 1) __syncthreads();
+  fft_line_plan<PL>(v, p, sm, tw);
+  // every thread read its part of the stage buffer before the first transform's barriers: reuse it for A
+#pragma unroll
+  for (int e = 0; e < E; ++e) stage[(p + P * e) * T + c] = cswap(v[e]);
+  fence_proxy_async();
+  if constexpr (!POISSON) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const float g = __ldg(grad + p + P * e);
+      const float2 a = park[e * (T * P)];
+      v[e] = make_float2(a.x * g, a.y * g);
+    }
+  }
+  __syncthreads();                                      // A staged (and the park slots read) by every thread
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_store_3d(&m_a, col0, y, x0 + b * BOXR, stage + b * BOXR * T);
+    tma_store_commit();
+  }
+  if constexpr (!POISSON) {
+    fft_line_plan<PL>(v, p, sm, tw);
+#pragma unroll
+    for (int e = 0; e < E; ++e) park_tile[(p + P * e) * T + c] = cswap(v[e]);
+    fence_proxy_async();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int b = 0; b < NBOX; ++b) tma_store_3d(&m_bx, col0, y, x0 + b * BOXR, park_tile + b * BOXR * T);
+      tma_store_commit();
+    }
+  }
+  if (threadIdx.x == 0) tma_store_wait_read();
 }
 
 // The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved

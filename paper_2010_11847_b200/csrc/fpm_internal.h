@@ -1,5 +1,6 @@
 // fpm_internal.h -- context and internal launch interfaces of libfpm (not part of the C-ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -82,6 +83,17 @@ void kernel_tables_destroy(KernelTables* t);
 // element-wise epilogue/prologue selectors for the fused x passes (fft.cu)
 enum XOp { XOP_NONE = 0, XOP_INVLAP = 1, XOP_GRAD = 2 };
 
+// TMA tensor maps of the four internal half-complex meshes of the fused paths (dk, wa, wb, wc; padded
+// pitch): `y` moves 16-column x 256-line boxes of one x slab, `x` moves TX-column boxes of 256 x lines.
+struct TileMaps {
+  bool ok = false;
+  CUtensorMap y[4];
+  CUtensorMap x[4];
+};
+// bufs: dk, wa, wb, wc (each `batch` meshes back to back).  Leaves out->ok false (and returns cudaSuccess)
+// when the driver has no tensor-map support: the callers then use the ld.global tile movers.
+cudaError_t fft_make_tile_maps(int n, int batch, float2* const bufs[4], TileMaps* out);
+
 cudaError_t fft_r2c(const FftTables& t, const float* real, float2* cplx, cudaStream_t s,
                     Profiler* prof = nullptr);
 cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t s,
@@ -93,11 +105,11 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
 // batch > 1 (F4 only): every buffer holds `batch` meshes back to back and each pass covers them all
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof = nullptr, int batch = 1);
+                            cudaStream_t s, Profiler* prof = nullptr, int batch = 1, const TileMaps* maps = nullptr);
 
 // out = c2r[(scale / K^2) r2c[src]] with the multiplier fused into the x round trip (backward pass)
 cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
-                        float scale, cudaStream_t s, Profiler* prof = nullptr);
+                        float scale, cudaStream_t s, Profiler* prof = nullptr, const CUtensorMap* work_map_x = nullptr);
 
 // ---- particle <-> mesh (mesh_ops.cu) ---------------------------------------------------------
 // How the caller's particle arrays are ordered: np > 0 says "n == np^3 particles in lattice
@@ -165,6 +177,13 @@ cudaError_t lpt_wrap(float* pos, int64_t n3, int ng, cudaStream_t s);
 cudaError_t lpt_source(float* s, const float* a, const float* b, const float* c, int64_t n, int mode,
                        cudaStream_t st);
 
+// ---- multi-grid pyramid (pyramid.cu, Alg. 2-3) --------------------------------
+// one REDUCE level n^3 -> (n/2)^3; tmp: 3 n^3 / 4 floats
+cudaError_t pyramid_reduce_level(const float* in, int n, float* tmp, float* out, cudaStream_t s);
+// one EXPAND level m^3 -> (2m)^3; tmp: 6 m^3 floats
+cudaError_t pyramid_expand_level(const float* in, int m, float* tmp, float* out, cudaStream_t s);
+cudaError_t pyramid_combine(float* fs, const float* up, const float* lowup, int64_t n, cudaStream_t s);
+
 // ---- MAP reconstruction element-wise kernels (recon.cu) ----------------------
 cudaError_t recon_residual(const float* rho, const float* data, float inv_s2, int64_t n, float* gbar,
                            double* acc, cudaStream_t s);
@@ -189,6 +208,10 @@ struct fpm_ctx {
   fpm::KernelTables kt_g, kt_p;     // transfer-function tables on ng; spectral tables on np
   void* ws = nullptr;
   size_t ws_bytes = 0;
+  fpm::TileMaps maps;               // tensor maps of the workspace's half-complex meshes (fpm_set_workspace)
+  int coarse_n = 0;                 // plans of the coarse mesh of the pyramid scheme (fpm_force_pyramid), made on demand
+  fpm::FftTables fft_c;
+  fpm::KernelTables kt_c;
   double* d_acc = nullptr;          // two float64 accumulators (loss terms of fpm_recon_loss_grad)
   bool sticky = false;
   std::string err;

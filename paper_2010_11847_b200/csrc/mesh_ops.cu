@@ -184,8 +184,8 @@ __device__ __forceinline__ void red_plane(unsigned addr, const V (&v)[4]) {
 // XMERGE (RES = 1): a thread's 8 particles are neighbours along x; when particle k+1 falls in the next x
 // plane of the same (y, z) cell column, its lower-plane deposits are added in registers to the upper-plane
 // deposits of particle k and go out as 4 reductions instead of 8.
-template <bool FIXED, bool HAS_MASS, int RES = 1, bool XMERGE = false>
-__global__ void __launch_bounds__(kBrickThreads, 2)
+template <bool FIXED, bool HAS_MASS, int RES = 1, bool XMERGE = false, int OCC = 2>
+__global__ void __launch_bounds__(kBrickThreads, OCC)
 paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass, float mass_const,
                    int64_t n, BrickMap bm, int ng, float* __restrict__ mesh) {
   constexpr int SX = BX / RES, SY = BY / RES, SZ = BZ / RES;          // lattice sites of the sub-brick
@@ -808,6 +808,7 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
   }
   if (mode == FPM_PAINT_BRICK_FIXED) {
     static const bool xmerge = !(std::getenv("FPM_TUNE_XMERGE") && std::getenv("FPM_TUNE_XMERGE")[0] == '0');
+    if (xmerge && !mass && tune("PAINT_OCC", 2) == 3) return go(paint_brick_kernel<true, false, 1, true, 3>);
     if (xmerge) return mass ? go(paint_brick_kernel<true, true, 1, true>) : go(paint_brick_kernel<true, false, 1, true>);
     return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
   }
