@@ -917,16 +917,21 @@ int fpm_force_pyramid(fpm_ctx* ctx, const float* pos, int64_t n, int levels, flo
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
   { ProfScope sc(pr, K_GREEN); FPM_CUDA(ctx, apply_force_kernel(ctx->kt_g, w.dk, scale, w.fk[0], w.fk[1], w.fk[2], s)); }
   for (int d = 0; d < 3; ++d) FPM_CUDA(ctx, fft_c2r(ctx->fft_g, w.fk[d], w.F[d], s, pr));
-  // the four half-complex regions are free now; each holds two real meshes
+  if (levels == 0) {     // no reduction: F_L = F_S and EXPAND = REDUCE = identity, so F = F_S exactly
+    ProfScope sc(pr, K_READOUT);
+    FPM_CUDA(ctx, readout3(w.F[0], w.F[1], w.F[2], pos, n, ng, force, order_of(ctx, n), s));
+    return FPM_OK;
+  }
+  // the four half-complex regions are free now; each holds one real mesh (and a little more: padded pitch)
   const int64_t g3 = cube(ng), c3 = cube(nc);
-  float* scratch = reinterpret_cast<float*>(w.dk);            // pyr_reduce / pyr_expand scratch (g3 floats)
-  float* up = reinterpret_cast<float*>(w.fk[0]);              // EXPAND(F_L)
-  float* lowup = up + g3;                                     // EXPAND(REDUCE(F_S))
-  float* coarse = reinterpret_cast<float*>(w.fk[1]);          // D | F_L[3] | low
+  float* scratch = reinterpret_cast<float*>(w.dk);            // pyr_reduce / pyr_expand scratch (< g3 floats)
+  float* up = w.rho;                                          // EXPAND(F_L): rho is dead once D is made
+  float* lowup = reinterpret_cast<float*>(w.fk[0]);           // EXPAND(REDUCE(F_S))
+  float* coarse = reinterpret_cast<float*>(w.fk[1]);          // D | F_L[3] | low   (5 c3 <= 5/8 g3 floats)
   float* D = coarse;
   float* FL[3] = {coarse + c3, coarse + 2 * c3, coarse + 3 * c3};
   float* low = coarse + 4 * c3;
-  float2* ck = reinterpret_cast<float2*>(w.fk[2]);            // coarse spectra: dk | fk[3]
+  float2* ck = reinterpret_cast<float2*>(w.fk[2]);            // coarse spectra: dk | fk[3]  (~4 c3 floats)
   const int64_t ckn = (int64_t)nc * nc * (nc / 2 + 1);
   // D <= REDUCE(H);  F_L <= ForceGrids(D, distributed), in fine-cell units
   int rc = pyr_reduce(ctx, w.rho, ng, levels, scratch, D);

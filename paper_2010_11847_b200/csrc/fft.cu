@@ -31,6 +31,7 @@ PlanInfo plan_info(int n) {
 // stage s >= 1: table[(t-1) NS + k] = exp(-2 pi i t k / (NS R_s)), t = 1..R_s-1, k < NS
 PlanInfo plan_info_x(int n) {      // plan of the fused x round trip (fft_x_force_kernel)
   if (n == 512) return Plan<512, 1>::info();
+  if (n == 1024) return Plan<1024, 1>::info();
   return plan_info(n);
 }
 
@@ -94,17 +95,28 @@ cudaError_t r2c_impl(const FftTables& t, const float* real, float2* cplx, cudaSt
 
 template <int N>
 cudaError_t launch_z_c2r(const FftTables& t, const float2* cplx, float* real, const float* gz,
-                         cudaStream_t s, Profiler* prof, int pitch = N / 2 + 1) {
+                         cudaStream_t s, Profiler* prof, int pitch = N / 2 + 1, int batch = 1) {
   constexpr int M = N / 2, G = z_rows<N>();
-  const int64_t nrows = (int64_t)N * N;
+  const int64_t nrows = (int64_t)N * N * batch;
   ProfScope sc(prof, K_FFT_Z_C2R);
   constexpr int threads = G * Plan<M>::P;
-  const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
-  auto kern = fft_z_c2r_kernel<N>;
-  cudaError_t e = set_smem(kern, smem);
-  if (e != cudaSuccess) return e;
   const float scale = (float)(1.0 / ((double)N * N * N));
-  kern<<<(unsigned)((nrows + G - 1) / G), threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz, pitch);
+  const unsigned grid = (unsigned)((nrows + G - 1) / G);
+  // bulk row loads need whole blocks of an even number of rows (16-byte aligned runs)
+  const bool tma = G % 2 == 0 && nrows % G == 0 && (reinterpret_cast<uintptr_t>(cplx) & 15) == 0 && tune("ZTMA", 1);
+  cudaError_t e;
+  if (tma) {
+    auto kern = fft_z_c2r_kernel<N, true>;
+    e = set_smem(kern, zc_smem_bytes<N>());
+    if (e != cudaSuccess) return e;
+    kern<<<grid, threads, zc_smem_bytes<N>(), s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz, pitch);
+  } else {
+    const size_t smem = Plan<M>::NST > 1 ? sizeof(float2) * G * row_pitch(M) : 0;
+    auto kern = fft_z_c2r_kernel<N, false>;
+    e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, threads, smem, s>>>(cplx, real, nrows, t.stage_m, t.full, scale, gz, pitch);
+  }
   return cudaGetLastError();
 }
 
@@ -140,7 +152,9 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
   const dim3 grid((nzh + TX - 1) / TX, N, batch);
   const unsigned threads = TX * Plan<N, xf_variant<N>()>::P;
   cudaError_t e;
-  if (m_in && m_a && (poisson || m_bx) && tune("TMA", 1)) {     // TMA tile movers
+  // (at N = 1024 the three-buffer tile is 192 KB, one block per SM, and the ld.global version with its two
+  //  64 KB buffers is faster: 6.1 vs 6.7 ms at C5)
+  if (m_in && m_a && (poisson || m_bx) && tune("TMA", N <= 512 ? 1 : 0)) {     // TMA tile movers
     const size_t smem = xf_tma_smem_bytes<N>();
     if (poisson) {
       auto kern = fft_x_force_tma_kernel<N, true>;
@@ -199,7 +213,22 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    e = launch_cols<N, false>(dk, dk, slabs, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
+    if (tma && tune("TMA", N <= 512 ? 1 : 0) && tune("YFWD_TMA", 1)) {
+      constexpr int TY = yi_tile<N>();
+      const size_t ysmem = sizeof(float2) * N * TY + 16;
+      dim3 grid((nzh + TY - 1) / TY, slabs);
+      auto go = [&](auto kern) {
+        e = set_smem(kern, ysmem);
+        if (e != cudaSuccess) return;
+        kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[0], maps->y[0], maps->y[0], maps->y[0],
+                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+        e = cudaGetLastError();
+      };
+      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 3 : 1)>);
+      else go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 2 : 1)>);
+    } else {
+      e = launch_cols<N, false>(dk, dk, slabs, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
+    }
     if (e != cudaSuccess) return e;
   }
   {
@@ -212,15 +241,19 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     ProfScope sc(prof, K_FFT_Y_INV3);
     using YPL = Plan<N, yi_variant<N>()>;
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    if (tma && tune("TMA", 1)) {
+    if (tma && tune("TMA", N <= 512 ? 1 : 0)) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = sizeof(float2) * N * TY + 16;
-      auto kern = fft_y_inv3_tma_kernel<N>;
-      e = set_smem(kern, ysmem);
-      if (e != cudaSuccess) return e;
       dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
-      kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
-                                                yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+      auto go = [&](auto kern) {
+        e = set_smem(kern, ysmem);
+        if (e != cudaSuccess) return;
+        kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
+                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+      };
+      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 3 : 1)>);
+      else go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 2 : 1)>);
+      if (e != cudaSuccess) return e;
     } else if (tune("YPAIR", 1)) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;

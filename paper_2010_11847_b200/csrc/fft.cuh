@@ -143,6 +143,7 @@ FPM_PLAN(256, 16, 2, 16, 16, 1)
 FPM_PLAN(512, 32, 2, 32, 16, 1)
 FPM_PLAN(1024, 32, 2, 32, 32, 1)
 FPM_PLAN_V(512, 1, 8, 3, 8, 8, 8)
+FPM_PLAN_V(1024, 1, 16, 3, 16, 8, 8)
 #undef FPM_PLAN
 #undef FPM_PLAN_V
 

@@ -17,6 +17,59 @@ struct OpNone {
   __device__ __forceinline__ float2 store(float2 v, int, int64_t, int) const { return v; }
 };
 
+// ---- TMA bulk copy + mbarrier (sm_90+/sm_100a) ------------------------------------------------------------
+// One elected thread arms the barrier with the byte count and issues cp.async.bulk; the copy engine writes
+// shared memory directly (no LSU data-pipe wavefronts, no registers) and completes the transaction count.
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+// global -> shared, bytes a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, uint64_t* bar) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(d), "l"(gsrc), "r"(bytes), "r"(b) : "memory");
+}
+
+// 3-D tiled tensor copies (cp.async.bulk.tensor): one instruction moves a box of up to 256 lines x 128 bytes
+// between a half-complex mesh (dims kz, y, x-slab; padded pitch) and a dense shared-memory tile.  Columns
+// beyond n/2 + 1 are out of bounds for the tensor map: zero-filled on load, dropped on store.
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint64_t* bar) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(d), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(b) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, int c0, int c1, int c2, const void* smem_src) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_src);
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(reinterpret_cast<uint64_t>(map)), "r"(sa), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes to shared memory -> visible to the async proxy (before a TMA store reads them)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int N> __host__ __device__ constexpr int tma_box_rows() { return N < 256 ? N : 256; }
+
 template <int N> __host__ __device__ constexpr int col_tile() { return N >= 64 ? 16 : 32; }
 // resident blocks per SM the column kernels are compiled for: at N = 512 the 64 KB tile allows three,
 // which needs <= 85 registers (the compiler otherwise settles just above and only two fit)
@@ -71,7 +124,7 @@ fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
 template <int N> __host__ __device__ constexpr int xf_tile() { return N >= 512 ? 8 : col_tile<N>(); }
 // plan variant of the x round trip: three transforms per tile make it compute-latency bound, so at
 // N = 512 it runs the 8-points-per-thread plan (32 instead of 12 resident warps per SM)
-template <int N> __host__ __device__ constexpr int xf_variant() { return N == 512 ? 1 : 0; }
+template <int N> __host__ __device__ constexpr int xf_variant() { return N >= 512 ? 1 : 0; }
 template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
   return sizeof(float2) * 2 * (size_t)N * xf_tile<N>();
 }
@@ -143,7 +196,7 @@ fft_x_force_kernel(const float2* in, float2* out_a,
 // lane, a tile line is 16 columns = one 128-byte line (the meshes have the padded pitch, a multiple of 16).
 // At N >= 512 it runs the 8-points-per-thread plan (16 complex values per thread for the pair).
 template <int N> __host__ __device__ constexpr int yi_tile() { return 16; }
-template <int N> __host__ __device__ constexpr int yi_variant() { return N == 512 ? 1 : 0; }
+template <int N> __host__ __device__ constexpr int yi_variant() { return N >= 512 ? 1 : 0; }
 template <int N> __host__ __device__ constexpr int yi_threads() { return (yi_tile<N>() / 2) * Plan<N, yi_variant<N>()>::P; }
 
 template <int N>
@@ -260,19 +313,41 @@ fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t
 }
 
 // rows of N/2+1 complex -> real rows of N floats, times `scale`.
-template <int N>
+// TMA: the block's G rows are one contiguous, 16-byte aligned run at any even G (dense or padded pitch), so
+// they arrive by one bulk copy and the Hermitian merge reads X[k], X[M-k] from shared memory (see
+// fft_z_c2r3_kernel); the caller uses it when nrows is a multiple of G.
+template <int N> __host__ __device__ constexpr int zc_row_pitch() {
+  return row_pitch(N / 2) > padded_pitch(N) ? row_pitch(N / 2) : padded_pitch(N);
+}
+template <int N> __host__ __device__ constexpr size_t zc_smem_bytes() {
+  return sizeof(float2) * (size_t)z_rows<N>() * zc_row_pitch<N>() + 16;
+}
+
+template <int N, bool TMA = false>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)
 fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t nrows,
                  const float2* __restrict__ tw, const float2* __restrict__ twn, float scale,
                  const float* __restrict__ gz, int in_pitch) {
-  extern __shared__ float2 smem[];
+  extern __shared__ __align__(128) float2 smem[];
   constexpr int M = N / 2;
   using PL = Plan<M>;
   constexpr int E = PL::E, P = PL::P, G = z_rows<N>();
   const int p = threadIdx.x % P, g = threadIdx.x / P;
-  const int64_t row = (int64_t)blockIdx.x * G + g;
+  const int64_t row0 = (int64_t)blockIdx.x * G, row = row0 + g;
   const bool ok = row < nrows;
   const float2* src = in + row * in_pitch;
+  if (TMA) {
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + G * zc_row_pitch<N>());
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const unsigned bytes = (unsigned)(sizeof(float2) * G * in_pitch);
+      mbar_expect_tx(bar, bytes);
+      bulk_load(smem, in + row0 * in_pitch, bytes, bar);
+    }
+    mbar_wait(bar, 0);
+    src = smem + g * in_pitch;
+  }
   float2 v[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) {
@@ -297,6 +372,7 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
     }
     v[e] = cswap(z);
   }
+  if (TMA) __syncthreads();            // the staged rows are in registers: the buffer becomes the exchange buffer
   RowSmem sm{smem + g * row_pitch(M)};
   fft_line<M>(v, p, sm, tw);
   if (!ok) return;
@@ -305,66 +381,16 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
   for (int e = 0; e < E; ++e) dst[p + P * e] = make_float2(v[e].y * scale, v[e].x * scale);
 }
 
-// ---- TMA bulk copy + mbarrier (sm_90+/sm_100a) ------------------------------------------------------------
-// One elected thread arms the barrier with the byte count and issues cp.async.bulk; the copy engine writes
-// shared memory directly (no LSU data-pipe wavefronts, no registers) and completes the transaction count.
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
-  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
-  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
-  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "MBAR_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra MBAR_DONE;\n"
-      "bra MBAR_WAIT;\n"
-      "MBAR_DONE:\n"
-      "}\n" ::"r"(a), "r"(parity) : "memory");
-}
-// global -> shared, bytes a multiple of 16, both addresses 16-byte aligned
-__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, uint64_t* bar) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(d), "l"(gsrc), "r"(bytes), "r"(b) : "memory");
-}
-
-// 3-D tiled tensor copies (cp.async.bulk.tensor): one instruction moves a box of up to 256 lines x 128 bytes
-// between a half-complex mesh (dims kz, y, x-slab; padded pitch) and a dense shared-memory tile.  Columns
-// beyond n/2 + 1 are out of bounds for the tensor map: zero-filled on load, dropped on store.
-__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2,
-                                            uint64_t* bar) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst), b = (unsigned)__cvta_generic_to_shared(bar);
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-      ::"r"(d), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(b) : "memory");
-}
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, int c0, int c1, int c2, const void* smem_src) {
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_src);
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
-               ::"l"(reinterpret_cast<uint64_t>(map)), "r"(sa), "r"(c0), "r"(c1), "r"(c2) : "memory");
-}
-__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-// generic-proxy writes to shared memory -> visible to the async proxy (before a TMA store reads them)
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-template <int N> __host__ __device__ constexpr int tma_box_rows() { return N < 256 ? N : 256; }
 
 // The three inverse y passes (see fft_y_inv3_pair_kernel) with the tiles moved by TMA: the whole 16-column
 // tile (N lines x 128 bytes) lands in shared memory with N / 256 tensor copies issued by one thread, the
 // transform runs register-resident out of it, the exchange reuses the same tile, and the result leaves by
 // TMA stores.  No global load or store goes through the LSU data pipe, which bounded the ld.global version
 // (profiles/r01_E: L1 data-pipe 85 %, 56 % of it global accesses).
-template <int N>
-__global__ void __launch_bounds__(yi_threads<N>())
+// INV3 = false: the plain forward y pass of the same meshes (in place through m_bx), one variant.
+// OCC: resident blocks per SM the kernel is compiled for (3 x 64 KB tiles fit at N = 512 with <= 42 registers).
+template <int N, bool INV3 = true, int OCC = 1>
+__global__ void __launch_bounds__(yi_threads<N>(), OCC)
 fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_constant__ CUtensorMap m_a,
                       const __grid_constant__ CUtensorMap m_y, const __grid_constant__ CUtensorMap m_z,
                       const float2* __restrict__ tw, const float* __restrict__ grad) {
@@ -373,7 +399,7 @@ fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_con
   constexpr int T = yi_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + N * T);
   const int c2 = threadIdx.x % (T / 2), p = threadIdx.x / (T / 2);
-  const int variant = blockIdx.x % 3, col0 = (blockIdx.x / 3) * T, slab = blockIdx.y;
+  const int variant = INV3 ? blockIdx.x % 3 : 0, col0 = (INV3 ? blockIdx.x / 3 : blockIdx.x) * T, slab = blockIdx.y;
   const CUtensorMap* in = variant == 0 ? &m_bx : &m_a;
   const CUtensorMap* out = variant == 0 ? &m_bx : (variant == 1 ? &m_y : &m_z);
   if (threadIdx.x == 0) mbar_init(bar, 1);
@@ -390,8 +416,9 @@ fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_con
   for (int e = 0; e < E; ++e) {
     const int i = p + P * e;
     float4 q = tile4[i * (T / 2) + c2];
-    if (variant == 1) { const float g = __ldg(grad + i); q.x *= g; q.y *= g; q.z *= g; q.w *= g; }
-    v[e] = cpair{make_float2(q.y, q.x), make_float2(q.w, q.z)};     // (im, re)-swapped: inverse transform
+    if (INV3 && variant == 1) { const float g = __ldg(grad + i); q.x *= g; q.y *= g; q.z *= g; q.w *= g; }
+    // inverse: (im, re)-swapped data through the forward butterflies
+    v[e] = INV3 ? cpair{make_float2(q.y, q.x), make_float2(q.w, q.z)} : cpair{make_float2(q.x, q.y), make_float2(q.z, q.w)};
   }
   if constexpr (PL::NST > 1) __syncthreads();       // the landed tile is in registers: it becomes the exchange buffer
   ColSmem2<T> sm{tile4, c2};
@@ -399,7 +426,8 @@ fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_con
   if constexpr (PL::NST > 1) __syncthreads();       // last exchange read: the tile becomes the output stage
 #pragma unroll
   for (int e = 0; e < E; ++e)
-    tile4[(p + P * e) * (T / 2) + c2] = make_float4(v[e].a.y, v[e].a.x, v[e].b.y, v[e].b.x);
+    tile4[(p + P * e) * (T / 2) + c2] = INV3 ? make_float4(v[e].a.y, v[e].a.x, v[e].b.y, v[e].b.x)
+                                             : make_float4(v[e].a.x, v[e].a.y, v[e].b.x, v[e].b.y);
   fence_proxy_async();
   __syncthreads();
   if (threadIdx.x == 0) {

@@ -808,7 +808,7 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
   }
   if (mode == FPM_PAINT_BRICK_FIXED) {
     static const bool xmerge = !(std::getenv("FPM_TUNE_XMERGE") && std::getenv("FPM_TUNE_XMERGE")[0] == '0');
-    if (xmerge && !mass && tune("PAINT_OCC", 2) == 3) return go(paint_brick_kernel<true, false, 1, true, 3>);
+    if (xmerge && !mass && tune("PAINT_OCC", 3) == 3) return go(paint_brick_kernel<true, false, 1, true, 3>);
     if (xmerge) return mass ? go(paint_brick_kernel<true, true, 1, true>) : go(paint_brick_kernel<true, false, 1, true>);
     return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
   }
