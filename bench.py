@@ -499,6 +499,7 @@ def main():
         kernels[name] = k
     dominant = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
     traffic_table, traffic_src = ncu_traffic(args.config)     # per-launch DRAM bytes from the committed ncu capture
+    late_table, late_src = ncu_traffic(args.config + "-late")   # the same at the clustered end of the schedule
     traffic = traffic_table.get(dominant)
     for name, k in kernels.items():
         if name in traffic_table:
@@ -508,6 +509,9 @@ def main():
                 "unit": "GB/s", "frac": dk.get("frac"), "traffic": traffic, "peak_source": peak_src,
                 "traffic_source": (f"profiles/ncu_traffic.csv, capture {traffic_src.get(dominant)} (an earlier ncu --set "
                                    f"full run of this command, not this run)") if traffic is not None else None,
+                "traffic_late": late_table.get(dominant),
+                "traffic_late_source": (f"profiles/ncu_traffic.csv, capture {late_src.get(dominant)}"
+                                        if late_table.get(dominant) is not None else None),
                 "share_of_step": dk["ms_per_step"] / ms_per_step}
     own, bound, unf = step_bytes_fused_path(n_p, ng), step_bytes_fused_bound(n_p, ng), step_bytes_unfused(n_p, ng)
     fused = args.force_path == "fused"

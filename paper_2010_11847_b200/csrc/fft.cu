@@ -221,7 +221,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
         e = set_smem(kern, ysmem);
         if (e != cudaSuccess) return;
         kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[0], maps->y[0], maps->y[0], maps->y[0],
-                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
         e = cudaGetLastError();
       };
       if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 3 : 1)>);
@@ -249,7 +249,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
         e = set_smem(kern, ysmem);
         if (e != cudaSuccess) return;
         kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
-                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
+                                                  yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
       };
       if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 3 : 1)>);
       else go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 2 : 1)>);

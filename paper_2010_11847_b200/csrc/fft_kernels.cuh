@@ -393,13 +393,14 @@ template <int N, bool INV3 = true, int OCC = 1>
 __global__ void __launch_bounds__(yi_threads<N>(), OCC)
 fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_constant__ CUtensorMap m_a,
                       const __grid_constant__ CUtensorMap m_y, const __grid_constant__ CUtensorMap m_z,
-                      const float2* __restrict__ tw, const float* __restrict__ grad) {
+                      const float2* __restrict__ tw, const float* __restrict__ grad, int slab0) {
   extern __shared__ __align__(128) float2 smem[];
   using PL = Plan<N, yi_variant<N>()>;
   constexpr int T = yi_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + N * T);
   const int c2 = threadIdx.x % (T / 2), p = threadIdx.x / (T / 2);
-  const int variant = INV3 ? blockIdx.x % 3 : 0, col0 = (INV3 ? blockIdx.x / 3 : blockIdx.x) * T, slab = blockIdx.y;
+  const int variant = INV3 ? blockIdx.x % 3 : 0, col0 = (INV3 ? blockIdx.x / 3 : blockIdx.x) * T,
+            slab = slab0 + blockIdx.y;
   const CUtensorMap* in = variant == 0 ? &m_bx : &m_a;
   const CUtensorMap* out = variant == 0 ? &m_bx : (variant == 1 ? &m_y : &m_z);
   if (threadIdx.x == 0) mbar_init(bar, 1);
@@ -523,7 +524,7 @@ fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_co
 
 // The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved
 // per cell as float4 (F_x, F_y, F_z, 0): the readout then needs one 16-byte gather per CIC corner
-// instead of three 4-byte ones (profiles/r01_B: the gather was request- and latency-bound).
+// instead of three 4-byte ones (round-1 ncu capture: the gather was request- and latency-bound).
 // A block owns GC rows; its three thread groups (GC*P threads each, whole warps) invert the rows of
 // component 0, 1, 2 concurrently, each with its own exchange buffer, park the real rows there, and
 // the block then writes its GC*N cells as fully coalesced float4.

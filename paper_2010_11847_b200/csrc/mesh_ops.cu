@@ -31,7 +31,7 @@ struct Cic {
 
 // floor / round-to-nearest without the conversion (XU) pipe: adding 1.5 * 2^23 leaves the integer in
 // the low mantissa bits.  Exact for |x| < 2^22, far beyond any position in mesh cells (ng <= 1024);
-// FRND/F2I issue at a quarter of the FMA rate and dominated the paint kernel (profiles/r01_A).
+// FRND/F2I issue at a quarter of the FMA rate and dominated the paint kernel in the first round-1 capture.
 constexpr float kMagic = 12582912.f;
 constexpr int kMagicBits = 0x4B400000;
 __device__ __forceinline__ float fast_rint(float x, int& i) {
@@ -376,7 +376,7 @@ paint_brick_kernel(const float* __restrict__ pos, const float* __restrict__ mass
 
 // ---- readout -----------------------------------------------------------------------------------
 // 32-bit cell indices (ng <= 1024: ng^3 <= 2^30), so every gather address is one IMAD.WIDE.U32; the
-// 64-bit row arithmetic was most of the instruction count of the readout kernels (profiles/r01_B).
+// 64-bit row arithmetic was most of the instruction count of the readout kernels in a round-1 capture.
 template <int NMESH>
 __device__ __forceinline__ void gather(const float* const* mesh, const Cic& c, unsigned g,
                                        float (&acc)[NMESH]) {

@@ -99,11 +99,52 @@ def big_run(name):
     print(f"[{name}] done {time.time() - t0:.0f} s", flush=True)
 
 
+def big_gradient(name):
+    """Float64 oracle gradient of BASELINE.json's backward objective at C3 size (configs[3] words it for C4, whose
+    float64 reverse run would take hours): L = sum(final density x seeded N(0,1) weight field, seed 101) with
+    respect to the linear field, through paint_adjoint -> nbody_vjp -> lpt_init_vjp (SURVEY.md 8(c) R12;
+    PAPER.md:21-23, 401, 586).  Stores the gradient at N_SAMPLE seeded lattice points and its 2-norm:
+      <name>_oracle_gradient.txt"""
+    import time
+    cfg = fi.CONFIGS[name]
+    om = fi.COSMO["omega_m"]
+    t0 = time.time()
+    delta = fi.linear_field(cfg.np_side, cfg.box, cfg.seed).astype(np.float64)
+    w = fi.weight_field(cfg.ng, 101).astype(np.float64)
+    mass = float(cfg.resolution_factor ** 3)
+    pos, mom = oracle.lpt_init(delta, cfg.ng, om, cfg.a0, cfg.lpt_order)
+    pf, _, traj = oracle.nbody(pos, mom, cfg.ng, cfg.np_side, om, cfg.stages(), return_traj=True)
+    del pos, mom
+    print(f"[{name} gradient] forward {time.time() - t0:.0f} s", flush=True)
+    loss = float(np.sum(oracle.paint(pf, cfg.ng, mass_const=mass) * w))
+    gx, _ = oracle.paint_adjoint(pf, cfg.ng, w, mass_const=mass)
+    del pf
+    gx0, gp0 = oracle.nbody_vjp(traj, cfg.ng, cfg.np_side, om, cfg.stages(), gx, np.zeros_like(gx))
+    del traj, gx
+    print(f"[{name} gradient] nbody_vjp {time.time() - t0:.0f} s", flush=True)
+    gd = oracle.lpt_init_vjp(delta, cfg.ng, om, cfg.a0, cfg.lpt_order, gx0, gp0)
+    idx = sample_indices(cfg.n_particles)
+    flat = gd.reshape(-1)
+    with open(os.path.join(HERE, f"{name.lower()}_oracle_gradient.txt"), "w") as f:
+        f.write(f"# float64 oracle: d/d(delta_lin) of L = sum(final density x weight field seed 101) for {name} "
+                f"({cfg.np_side}^3 particles on a {cfg.ng}^3 mesh, {cfg.n_steps} steps), SURVEY.md 8(c) R12.\n"
+                f"# Written by `python tests/golden/make_golden.py --config {name} --gradient` (calls only oracle/ and fpm_inputs/).\n"
+                f"# norms: loss {loss:.12e} grad_l2 {float(np.sqrt(np.sum(gd ** 2))):.12e} grad_maxabs {float(np.max(np.abs(gd))):.12e}\n"
+                "# flat_lattice_index gradient\n")
+        for i in idx:
+            f.write(f"{i} {flat[i]:.12e}\n")
+    print(f"[{name} gradient] done {time.time() - t0:.0f} s", flush=True)
+
+
 def main():
     import argparse
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", default=None, choices=["C3", "C4"])
+    ap.add_argument("--gradient", action="store_true", help="the reverse-mode gradient of the C4 objective at this config")
     args = ap.parse_args()
+    if args.config and args.gradient:
+        big_gradient(args.config)
+        return
     if args.config:
         big_run(args.config)
         return
