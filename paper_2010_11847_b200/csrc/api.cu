@@ -34,7 +34,8 @@ bool config_ok(const fpm_config* c) {
   return true;
 }
 
-const size_t kSkew = (size_t)256 * (size_t)tune("SKEW256", 37);   // bytes between consecutive half-complex buffers
+// bytes between consecutive half-complex buffers (A/B knob; measured to make no difference, so 0)
+const size_t kSkew = (size_t)256 * (size_t)tune("SKEW256", 0);
 
 inline int batch_of(const fpm_config& c) { return c.batch > 1 ? c.batch : 1; }
 
@@ -61,9 +62,8 @@ Workspace carve(const fpm_ctx* ctx) {
   const size_t b = (size_t)batch_of(ctx->cfg);
   w.rho = reinterpret_cast<float*>(p); p += b * real_bytes(n);
   for (int d = 0; d < 3; ++d) { w.F[d] = reinterpret_cast<float*>(p); p += b * real_bytes(n); }
-  // the four half-complex buffers are streamed concurrently at the same relative offset by the fused passes;
-  // their size is a large power of two times 17 or 33, so without a skew all streams fall on the same DRAM
-  // channels (measured: fft_z_c2r3 0.85 -> 1.02 ms with unskewed 128-byte-pitch buffers)
+  // (the four half-complex buffers are streamed concurrently at the same relative offset by the fused passes;
+  //  a skew between them was measured to make no difference: DESIGN.md section 15)
   w.dk = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew;
   for (int d = 0; d < 3; ++d) { w.fk[d] = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew; }
   return w;

@@ -446,13 +446,14 @@ template <int N> __host__ __device__ constexpr size_t xf_tma_smem_bytes() {
   return sizeof(float2) * 3 * (size_t)N * xf_tile<N>() + 16;
 }
 
-template <int N, bool POISSON = false>
-__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
+// VAR: plan variant (xf_variant<N>() by default; 0 = the 32-points-per-thread, one-exchange plan)
+template <int N, bool POISSON = false, int VAR = xf_variant<N>()>
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, VAR>::P, N == 512 ? 2 : 1)
 fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
                        const __grid_constant__ CUtensorMap m_bx, const float2* __restrict__ tw,
                        const float* __restrict__ lap, const float* __restrict__ grad, float scale) {
   extern __shared__ __align__(128) float2 smem[];
-  using PL = Plan<N, xf_variant<N>()>;
+  using PL = Plan<N, VAR>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
   float2* xch = smem;
   float2* park_tile = smem + N * T;

@@ -285,3 +285,43 @@ def test_C5_full_run_grows_the_largest_scales_linearly(c5, oracle):
           f"median |mode ratio| {np.median(ratios):.4f} over {len(ratios)} modes")
     assert growth == pytest.approx(d1, rel=0.02)
     assert np.median(ratios) == pytest.approx(d1, rel=0.03)
+
+
+def test_C3_gradient_lands_on_the_stored_oracle_gradient(fpm):
+    """BASELINE.json configs[3] asks for 'the backward pass: gradient of sum(final density x a seeded Gaussian
+    weight field) with respect to the initial linear modes, via adjoint paint/readout/FFT'.  The float64 reverse
+    run of C4 itself would take hours, so the oracle's gradient is stored at C3 size (256^3 particles on a 512^3
+    mesh, 10 steps; tests/golden/c3_oracle_gradient.txt, written by make_golden.py --config C3 --gradient) and the
+    GPU chain paint_adjoint -> fpm_nbody_vjp -> fpm_lpt_init_vjp must land on it.  Tolerance: relative 1e-3 of the
+    gradient's rms over the sample (the GPU differentiates along its own fp32 trajectory; same bound as the C1
+    test in test_gpu_backward.py); C4 itself keeps the finite-difference check of test_gpu_fullsize.py."""
+    import torch
+    path = os.path.join(GOLD, "c3_oracle_gradient.txt")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/c3_oracle_gradient.txt not generated")
+    cfg = fi.CONFIGS["C3"]
+    gold = _gold("c3_oracle_gradient.txt")
+    norms = _gold_norms("c3_oracle_gradient.txt")
+    n, stages = cfg.n_particles, cfg.stages()
+    torch.cuda.empty_cache()
+    ctx = fpm.FPM(cfg.ng, cfg.np_side, omega_m=OM, box=cfg.box, force_path=fpm.FORCE_FUSED)
+    delta = torch.from_numpy(fi.linear_field(cfg.np_side, cfg.box, cfg.seed)).cuda()
+    w = torch.from_numpy(fi.weight_field(cfg.ng, 101)).cuda()
+    pos, mom = ctx.lpt_init(delta, cfg.a0, cfg.lpt_order)
+    traj = torch.empty(cfg.n_steps + 1, 3, n, device="cuda")
+    ctx.nbody(pos, mom, stages, traj=traj)
+    loss = float((ctx.paint(pos).double() * w.double()).sum())
+    assert loss == pytest.approx(norms["loss"], rel=1e-3, abs=1e-3 * norms["grad_l2"])
+    gx, _ = ctx.paint_adjoint(pos, w, want_grad_mass=False)
+    gp = torch.zeros_like(gx)
+    ctx.nbody_vjp(traj, stages, gx, gp, grad_mom_is_zero=True)
+    gd = ctx.lpt_init_vjp(delta, cfg.a0, cfg.lpt_order, gx, gp)
+    got = host(gd.view(-1)[torch.from_numpy(gold[:, 0].astype(np.int64)).cuda()]).astype(np.float64)
+    ref = gold[:, 1]
+    err = np.abs(got - ref)
+    rms = norms["grad_l2"] / np.sqrt(n)
+    print(f"C3 gradient: sample rel-L2 {np.linalg.norm(got - ref) / np.linalg.norm(ref):.2e}, max-abs error {err.max():.2e} "
+          f"(gradient rms {rms:.2e}, max {norms['grad_maxabs']:.2e}); |grad|_2 GPU {float(torch.linalg.vector_norm(gd.double())):.6e} "
+          f"oracle {norms['grad_l2']:.6e}")
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 1e-3
+    assert float(torch.linalg.vector_norm(gd.double())) == pytest.approx(norms["grad_l2"], rel=1e-3)
