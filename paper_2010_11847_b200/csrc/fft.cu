@@ -156,13 +156,6 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
   //  64 KB buffers is faster: 6.1 vs 6.7 ms at C5)
   if (m_in && m_a && (poisson || m_bx) && tune("TMA", N <= 512 ? 1 : 0)) {     // TMA tile movers
     const size_t smem = xf_tma_smem_bytes<N>();
-    if (N == 512 && !poisson && tune("XVAR", 1) == 0) {      // experiment: one-exchange plan, 128 threads
-      auto kern = fft_x_force_tma_kernel<N, false, 0>;
-      e = set_smem(kern, smem);
-      if (e != cudaSuccess) return e;
-      kern<<<grid, TX * Plan<N, 0>::P, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_n, kt.lap, kt.grad, scale);
-      return cudaGetLastError();
-    }
     if (poisson) {
       auto kern = fft_x_force_tma_kernel<N, true>;
       e = set_smem(kern, smem);

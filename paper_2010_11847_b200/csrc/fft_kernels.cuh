@@ -446,7 +446,8 @@ template <int N> __host__ __device__ constexpr size_t xf_tma_smem_bytes() {
   return sizeof(float2) * 3 * (size_t)N * xf_tile<N>() + 16;
 }
 
-// VAR: plan variant (xf_variant<N>() by default; 0 = the 32-points-per-thread, one-exchange plan)
+// VAR: plan variant.  (The 32-points-per-thread, one-exchange plan Plan<512, 0> halves the shared-memory
+// traffic but leaves 8 warps per SM: 0.617 vs 0.522 ms.)
 template <int N, bool POISSON = false, int VAR = xf_variant<N>()>
 __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, VAR>::P, N == 512 ? 2 : 1)
 fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
