@@ -51,6 +51,12 @@ inline cudaError_t ensure_dynamic_smem(K kernel, size_t bytes) {
   return ensure_dynamic_smem_impl(reinterpret_cast<const void*>(kernel), bytes);
 }
 
+// cuTensorMapEncodeTiled through cudaGetDriverEntryPoint (no libcuda link); nullptr when unavailable (profiler.cpp)
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn();
+
 // Tuning switches for A/B measurements (environment FPM_TUNE_<NAME>, read once); the defaults are the
 // measured winners and the product never depends on a switch being set.
 int tune(const char* name, int dflt);     // profiler.cpp
