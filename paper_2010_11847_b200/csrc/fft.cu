@@ -213,7 +213,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    if (tma && tune("TMA", N <= 512 ? 1 : 0) && tune("YFWD_TMA", 1)) {
+    if (tma && tune("TMA", 1) && tune("YFWD_TMA", 1)) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = sizeof(float2) * N * TY + 16;
       dim3 grid((nzh + TY - 1) / TY, slabs);
@@ -241,7 +241,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     ProfScope sc(prof, K_FFT_Y_INV3);
     using YPL = Plan<N, yi_variant<N>()>;
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    if (tma && tune("TMA", N <= 512 ? 1 : 0)) {
+    if (tma && tune("TMA", 1)) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = sizeof(float2) * N * TY + 16;
       dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);

@@ -121,7 +121,13 @@ fft_cols_kernel(const float2* in, float2* out, int64_t batch_stride, int ncols,
 // while its inverse runs, so the forward transform is done once (1 forward + 2 inverse per column).
 // columns = flattened (y, kz), lines = x with stride line_stride; no normalisation here.
 // Tile of TX columns; shared memory = [exchange N*TX | parked spectrum N*TX] float2.
-template <int N> __host__ __device__ constexpr int xf_tile() { return N >= 512 ? 8 : col_tile<N>(); }
+#ifndef FPM_XF_TILE_1024
+#define FPM_XF_TILE_1024 8
+#endif
+#ifndef FPM_YI_TILE_1024
+#define FPM_YI_TILE_1024 8
+#endif
+template <int N> __host__ __device__ constexpr int xf_tile() { return N >= 1024 ? FPM_XF_TILE_1024 : (N >= 512 ? 8 : col_tile<N>()); }
 // plan variant of the x round trip: three transforms per tile make it compute-latency bound, so at
 // N = 512 it runs the 8-points-per-thread plan (32 instead of 12 resident warps per SM)
 template <int N> __host__ __device__ constexpr int xf_variant() { return N >= 512 ? 1 : 0; }
@@ -195,7 +201,7 @@ fft_x_force_kernel(const float2* in, float2* out_a,
 // A thread transforms a PAIR of adjacent columns (cpair): every global and shared access is 16 bytes per
 // lane, a tile line is 16 columns = one 128-byte line (the meshes have the padded pitch, a multiple of 16).
 // At N >= 512 it runs the 8-points-per-thread plan (16 complex values per thread for the pair).
-template <int N> __host__ __device__ constexpr int yi_tile() { return 16; }
+template <int N> __host__ __device__ constexpr int yi_tile() { return N >= 1024 ? 8 : 16; }
 template <int N> __host__ __device__ constexpr int yi_variant() { return N >= 512 ? 1 : 0; }
 template <int N> __host__ __device__ constexpr int yi_threads() { return (yi_tile<N>() / 2) * Plan<N, yi_variant<N>()>::P; }
 
