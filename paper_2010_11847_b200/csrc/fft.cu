@@ -224,7 +224,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
                                                   yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
         e = cudaGetLastError();
       };
-      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 3 : 1)>);
+      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 6 : 1)>);
       else go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 2 : 1)>);
     } else {
       e = launch_cols<N, false>(dk, dk, slabs, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
@@ -251,7 +251,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
         kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
                                                   yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
       };
-      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 3 : 1)>);
+      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 6 : 1)>);
       else go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 2 : 1)>);
       if (e != cudaSuccess) return e;
     } else if (tune("YPAIR", 1)) {

@@ -200,8 +200,8 @@ fft_x_force_kernel(const float2* in, float2* out_a,
 // by the z pass).  in0/out0 may alias; A is read by variants 1 and 2 and written by neither.
 // A thread transforms a PAIR of adjacent columns (cpair): every global and shared access is 16 bytes per
 // lane, a tile line is 16 columns = one 128-byte line (the meshes have the padded pitch, a multiple of 16).
-// At N >= 512 it runs the 8-points-per-thread plan (16 complex values per thread for the pair).
-template <int N> __host__ __device__ constexpr int yi_tile() { return N >= 1024 ? 8 : 16; }
+// At N >= 512 it runs the 8/16-points-per-thread plan variant and 8-column tiles (64-byte lines; 32 / 64 KB).
+template <int N> __host__ __device__ constexpr int yi_tile() { return N >= 512 ? 8 : 16; }
 template <int N> __host__ __device__ constexpr int yi_variant() { return N >= 512 ? 1 : 0; }
 template <int N> __host__ __device__ constexpr int yi_threads() { return (yi_tile<N>() / 2) * Plan<N, yi_variant<N>()>::P; }
 
