@@ -161,6 +161,11 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
       kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_a, t.stage_x, kt.lap, kt.grad, scale);
+    } else if (tune("XPAIR", 1)) {
+      auto kern = fft_x_force_pair_tma_kernel<N>;
+      e = set_smem(kern, smem);
+      if (e != cudaSuccess) return e;
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
     } else {
       auto kern = fft_x_force_tma_kernel<N, false>;
       e = set_smem(kern, smem);

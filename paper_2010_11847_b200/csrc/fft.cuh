@@ -161,6 +161,18 @@ struct ColSmem {
   __device__ __forceinline__ void st(int i, float2 x) const { base[line(i) * T + c] = x; }
   __device__ __forceinline__ float2 ld(int i) const { return base[line(i) * T + c]; }
 };
+// a tile whose elements are pairs (two spectra of the SAME column, 16 bytes): element i of column c at
+// i*T + c; with T = 8 a line is 128 bytes, all 32 banks
+template <int T>
+struct ColSmemQ {
+  float4* base;
+  int c;
+  __device__ __forceinline__ void st(int i, cpair x) const { base[i * T + c] = make_float4(x.a.x, x.a.y, x.b.x, x.b.y); }
+  __device__ __forceinline__ cpair ld(int i) const {
+    const float4 q = base[i * T + c];
+    return cpair{make_float2(q.x, q.y), make_float2(q.z, q.w)};
+  }
+};
 // the same tile accessed as column pairs: pair c2 of line i is one 16-byte word (T = 16: a line is 128 bytes)
 template <int T>
 struct ColSmem2 {

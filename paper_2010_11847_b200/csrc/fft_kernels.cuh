@@ -530,6 +530,72 @@ fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_co
   if (threadIdx.x == 0) tma_store_wait_read();
 }
 
+// The same round trip with the two inverse transforms run TOGETHER as one transform of pairs
+// (A, g(w_x) A): the pair lives in registers, so the spectrum is never parked in shared memory, the two
+// inverses share their barriers, and the pair exchange moves 16 bytes per element in 128-byte tile lines
+// (conflict-free, unlike the 64-byte lines of the 8-column complex tile).  15 instead of 17 passes over the
+// tile through the L1 data pipe, which bounds this kernel (profiles/r02_C4.md: 79 %).
+// Shared memory = [pair exchange 2 N T | stage N T] complex + the barrier (the same 96 KB at N = 512).
+template <int N>
+__global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
+fft_x_force_pair_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
+                            const __grid_constant__ CUtensorMap m_bx, const float2* __restrict__ tw,
+                            const float* __restrict__ lap, const float* __restrict__ grad, float scale) {
+  extern __shared__ __align__(128) float2 smem[];
+  using PL = Plan<N, xf_variant<N>()>;
+  constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
+  float2* xch = smem;                                   // 2 N T complex: forward exchange, pair exchange, B_x stage
+  float2* stage = smem + 2 * N * T;                     // N T complex: input tile, then A stage
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + 3 * N * T);
+  const int c = threadIdx.x % T, p = threadIdx.x / T;
+  const int y = blockIdx.y, col0 = blockIdx.x * T, kz = col0 + c, x0 = blockIdx.z * N;
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(bar, (unsigned)(sizeof(float2) * N * T));
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_load_3d(stage + b * BOXR * T, &m_in, col0, y, x0 + b * BOXR, bar);
+  }
+  mbar_wait(bar, 0);
+  cpair w[E];
+  {
+    float2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = stage[(p + P * e) * T + c];
+    ColSmem<T> sm{xch, c};
+    fft_line_plan<PL>(v, p, sm, tw);
+    const float lyz = __ldg(lap + y) + __ldg(lap + (kz <= N / 2 ? kz : 0));
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int i = p + P * e;
+      const float k2 = __ldg(lap + i) + lyz;
+      const float f = ((y | kz | i) == 0) ? 0.f : scale / k2;
+      const float g = __ldg(grad + i);
+      const float2 a = make_float2(v[e].x * f, -v[e].y * f);       // i f v, (im, re)-swapped
+      w[e] = cpair{a, make_float2(a.x * g, a.y * g)};
+    }
+  }
+  if constexpr (PL::NST > 1) __syncthreads();           // the forward exchange is read: reuse it for the pairs
+  ColSmemQ<T> smq{reinterpret_cast<float4*>(xch), c};
+  fft_line_plan<PL>(w, p, smq, tw);
+  if constexpr (PL::NST > 1) __syncthreads();           // the last pair exchange is read: B_x is staged over it
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    stage[(p + P * e) * T + c] = cswap(w[e].a);
+    xch[(p + P * e) * T + c] = cswap(w[e].b);
+  }
+  fence_proxy_async();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_store_3d(&m_a, col0, y, x0 + b * BOXR, stage + b * BOXR * T);
+#pragma unroll
+    for (int b = 0; b < NBOX; ++b) tma_store_3d(&m_bx, col0, y, x0 + b * BOXR, xch + b * BOXR * T);
+    tma_store_commit();
+    tma_store_wait_read();
+  }
+}
+
 // The three c2r z passes of the fused force path in one launch, writing the force mesh interleaved
 // per cell as float4 (F_x, F_y, F_z, 0): the readout then needs one 16-byte gather per CIC corner
 // instead of three 4-byte ones (round-1 ncu capture: the gather was request- and latency-bound).
