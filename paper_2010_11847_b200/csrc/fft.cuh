@@ -147,6 +147,11 @@ FPM_PLAN_V(1024, 1, 16, 3, 16, 8, 8)
 #undef FPM_PLAN
 #undef FPM_PLAN_V
 
+#ifndef FPM_TW_POW
+#define FPM_TW_POW 1
+#endif
+constexpr bool kTwiddlePowers = FPM_TW_POW != 0;
+
 // shared-memory accessors -----------------------------------------------------------------
 // column tile: element i of column c at i*T + c.  With T = 16 a line of the tile is 128 bytes, all 32 banks:
 // conflict-free by construction.  With T = 8 a line is 64 bytes, half the banks, and the two lines a
@@ -211,8 +216,22 @@ __device__ __forceinline__ void fft_stage(C (&v)[PL::E], const int p, const SM& 
     for (int t = 0; t < R; ++t) a[t] = v[u + t * M];
     if constexpr (NS > 1) {
       const float2* __restrict__ tws = tw + PL::toff(S) + k;
+      if constexpr (kTwiddlePowers && R >= 4) {
+        // only w^1, w^2, w^4, ... are loaded (correctly rounded table entries); w^t for the other t is one
+        // complex product of two entries already at hand: the loads go through the same L1 data pipe as the
+        // shared-memory exchanges that bound these kernels, the products through the idle FMA pipe
+        float2 w[R];
 #pragma unroll
-      for (int t = 1; t < R; ++t) a[t] = cmul(a[t], __ldg(tws + (t - 1) * NS));
+        for (int t = 1; t < R; ++t) {
+          if ((t & (t - 1)) == 0) w[t] = __ldg(tws + (t - 1) * NS);
+          else w[t] = cmul(w[t & (t - 1)], w[t & -t]);
+        }
+#pragma unroll
+        for (int t = 1; t < R; ++t) a[t] = cmul(a[t], w[t]);
+      } else {
+#pragma unroll
+        for (int t = 1; t < R; ++t) a[t] = cmul(a[t], __ldg(tws + (t - 1) * NS));
+      }
     }
     Dft<R>::apply(a);
     if constexpr (last) {
