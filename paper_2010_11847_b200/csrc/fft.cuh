@@ -40,42 +40,58 @@ __device__ __forceinline__ cpair csub(cpair x, cpair y) { return cpair{csub(x.a,
 __device__ __forceinline__ cpair cmul(cpair x, float2 w) { return cpair{cmul(x.a, w), cmul(x.b, w)}; }
 __device__ __forceinline__ cpair cswap(cpair x) { return cpair{cswap(x.a), cswap(x.b)}; }
 
-// cos(2 pi k / 32), k = 0..8
-__host__ __device__ constexpr float cos32_table(int k) {
-  constexpr float c[9] = {1.0f,
-                          0.98078528040323044913f,
-                          0.92387953251128675613f,
-                          0.83146961230254523708f,
-                          0.70710678118654752440f,
-                          0.55557023301960222474f,
-                          0.38268343236508977173f,
-                          0.19509032201612826785f,
-                          0.0f};
+// cos(2 pi k / 64), k = 0..16 (correctly rounded)
+__host__ __device__ constexpr float cos64_table(int k) {
+  constexpr float c[17] = {1.0f,
+                           0.995184726672196886245f,
+                           0.980785280403230449126f,
+                           0.956940335732208864936f,
+                           0.923879532511286756128f,
+                           0.881921264348355029713f,
+                           0.831469612302545237079f,
+                           0.773010453362736960811f,
+                           0.707106781186547524401f,
+                           0.634393284163645498215f,
+                           0.555570233019602224743f,
+                           0.471396736825997648556f,
+                           0.382683432365089771728f,
+                           0.290284677254462367636f,
+                           0.195090322016128267848f,
+                           0.0980171403295606019942f,
+                           0.0f};
   return c[k];
 }
-__host__ __device__ constexpr float cos32(int k) {
-  k = ((k % 32) + 32) % 32;
-  if (k > 16) k = 32 - k;
-  return k > 8 ? -cos32_table(16 - k) : cos32_table(k);
+__host__ __device__ constexpr float cos64(int k) {
+  k = ((k % 64) + 64) % 64;
+  if (k > 32) k = 64 - k;
+  return k > 16 ? -cos64_table(32 - k) : cos64_table(k);
 }
-__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+__host__ __device__ constexpr float sin64(int k) { return cos64(k - 16); }
 
-// x * exp(-2 pi i I / R), resolved at compile time
+// x * exp(-2 pi i I / R), resolved at compile time (R a power of two <= 64)
 template <int R, int I>
 __device__ __forceinline__ float2 mul_twiddle(float2 x);
 template <int R, int I>
 __device__ __forceinline__ cpair mul_twiddle(cpair x) { return cpair{mul_twiddle<R, I>(x.a), mul_twiddle<R, I>(x.b)}; }
 template <int R, int I>
 __device__ __forceinline__ float2 mul_twiddle(float2 x) {
-  constexpr int k = (I * (32 / R)) % 32;
+  constexpr int k = (I * (64 / R)) % 64;
   if constexpr (k == 0) return x;
-  else if constexpr (k == 8) return make_float2(x.y, -x.x);
-  else if constexpr (k == 16) return make_float2(-x.x, -x.y);
-  else if constexpr (k == 24) return make_float2(-x.y, x.x);
+  else if constexpr (k == 16) return make_float2(x.y, -x.x);
+  else if constexpr (k == 32) return make_float2(-x.x, -x.y);
+  else if constexpr (k == 48) return make_float2(-x.y, x.x);
   else {
-    constexpr float c = cos32(k), s = -sin32(k);
+    constexpr float c = cos64(k), s = -sin64(k);
     return make_float2(x.x * c - x.y * s, x.x * s + x.y * c);
   }
+}
+
+// w[e] = w0 * exp(-2 pi i e / R), e < sizeof...(I): the twiddles W_N^(p + P e) of the real-transform split /
+// merge from ONE table entry W_N^p (N = 2 E P, so W_N^(P e) = exp(-2 pi i e / (2 E)) is a compile-time constant);
+// E - 1 table loads less per thread through the L1 data pipe that bounds the z passes.
+template <int R, int... I>
+__device__ __forceinline__ void twiddle_ladder(float2 w0, float2 (&w)[sizeof...(I)], std::integer_sequence<int, I...>) {
+  ((w[I] = mul_twiddle<R, I>(w0)), ...);
 }
 
 // In-register forward DFT of R points (decimation in frequency), natural-order output.
@@ -178,7 +194,26 @@ struct ColSmemQ {
     return cpair{make_float2(q.x, q.y), make_float2(q.z, q.w)};
   }
 };
+// Exchange-buffer swizzle for tiles whose lines are 64 bytes (half the banks): line i sits at i ^ bit B of i.
+// Two lines a quarter-/half-warp touches together are either neighbours (i, i + 1: they keep opposite halves,
+// both flipped or neither) or R0 apart in the first stage's stores (lines R0 p + t of threads p, p + 1: with
+// B = log2 R0 exactly one of them flips).  Enumerated over every exchange access of the plans in use: 1.25-1.5
+// wavefronts per ideal one without it, 1.0 with it.  Used by the forward exchange of the x round trip
+// (fft_x_force 0.467 -> 0.456 ms).
+template <int B>
+__device__ __forceinline__ int swz_line(int i) { return B > 0 ? (i ^ ((i >> B) & 1)) : i; }
+__host__ __device__ constexpr int ilog2_c(int v) { return v <= 1 ? 0 : 1 + ilog2_c(v / 2); }
+// a column tile of single elements with the bit swizzle (T = 8: 64-byte lines)
+template <int T, int B>
+struct ColSmemB {
+  float2* base;
+  int c;
+  __device__ __forceinline__ void st(int i, float2 x) const { base[swz_line<B>(i) * T + c] = x; }
+  __device__ __forceinline__ float2 ld(int i) const { return base[swz_line<B>(i) * T + c]; }
+};
 // the same tile accessed as column pairs: pair c2 of line i is one 16-byte word (T = 16: a line is 128 bytes)
+// (with T = 8 the bit swizzle removes the 1.33 x STS.128 conflicts of fft_y_inv3 as well, but its address
+// arithmetic does not fit the 40 registers of 6 blocks/SM: 0.461 ms at 5 blocks/SM against 0.452 without)
 template <int T>
 struct ColSmem2 {
   float4* base;

@@ -300,6 +300,8 @@ fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t
   __syncthreads();
   if (!ok) return;
   float2* dst = out + row * out_pitch;
+  float2 wn[E];
+  twiddle_ladder<2 * E>(__ldg(twn + p), wn, std::make_integer_sequence<int, E>{});
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int k = p + P * e;
@@ -313,7 +315,7 @@ fft_z_r2c_kernel(const float* __restrict__ in, float2* __restrict__ out, int64_t
       const float2 xe = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
       const float2 d = make_float2(0.5f * (zk.x - zm.x), 0.5f * (zk.y + zm.y));
       const float2 xo = make_float2(d.y, -d.x);
-      dst[k] = cadd(xe, cmul(__ldg(twn + k), xo));
+      dst[k] = cadd(xe, cmul(wn[e], xo));
     }
   }
 }
@@ -354,7 +356,8 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
     mbar_wait(bar, 0);
     src = smem + g * in_pitch;
   }
-  float2 v[E];
+  float2 v[E], wn[E];
+  twiddle_ladder<2 * E>(__ldg(twn + p), wn, std::make_integer_sequence<int, E>{});
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int k = p + P * e;
@@ -371,7 +374,7 @@ fft_z_c2r_kernel(const float2* __restrict__ in, float* __restrict__ out, int64_t
         // A = X[k] + conj X[M-k], B = (X[k] - conj X[M-k]) exp(+2 pi i k/N), Z = A + i B
         const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
         const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
-        const float2 w = __ldg(twn + k);
+        const float2 w = wn[e];
         const float2 b = cmul(d, make_float2(w.x, -w.y));
         z = make_float2(a.x - b.y, a.y + b.x);
       }
@@ -562,7 +565,7 @@ fft_x_force_pair_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __gr
     float2 v[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = stage[(p + P * e) * T + c];
-    ColSmem<T> sm{xch, c};
+    ColSmemB<T, T == 8 ? ilog2_c(PL::R0) : 0> sm{xch, c};   // 64-byte lines: swizzled
     fft_line_plan<PL>(v, p, sm, tw);
     const float lyz = __ldg(lap + y) + __ldg(lap + (kz <= N / 2 ? kz : 0));
 #pragma unroll
@@ -649,7 +652,8 @@ fft_z_c2r3_kernel(const float2* __restrict__ in0, const float2* __restrict__ in1
     mbar_wait(bar, 0);
   }
   const float2* src = TMA ? region + g * PZ : (comp == 0 ? in0 : (comp == 1 ? in1 : in2)) + row * PZ;
-  float2 v[E];
+  float2 v[E], wn[E];
+  twiddle_ladder<2 * E>(__ldg(twn + p), wn, std::make_integer_sequence<int, E>{});
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int k = p + P * e;
@@ -664,7 +668,7 @@ fft_z_c2r3_kernel(const float2* __restrict__ in0, const float2* __restrict__ in1
     } else {
       const float2 a = make_float2(xk.x + xm.x, xk.y - xm.y);
       const float2 d = make_float2(xk.x - xm.x, xk.y + xm.y);
-      const float2 w = __ldg(twn + k);
+      const float2 w = wn[e];
       const float2 b = cmul(d, make_float2(w.x, -w.y));
       z = make_float2(a.x - b.y, a.y + b.x);
     }
