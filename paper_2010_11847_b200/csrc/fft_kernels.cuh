@@ -537,7 +537,7 @@ fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_co
 // (A, g(w_x) A): the pair lives in registers, so the spectrum is never parked in shared memory, the two
 // inverses share their barriers, and the pair exchange moves 16 bytes per element in 128-byte tile lines
 // (conflict-free, unlike the 64-byte lines of the 8-column complex tile).  15 instead of 17 passes over the
-// tile through the L1 data pipe, which bounds this kernel (profiles/r02_C4.md: 79 %).
+// tile through the L1 data pipe, which bounds this kernel (profiles/r02_final_C4.md: 79 %).
 // Shared memory = [pair exchange 2 N T | stage N T] complex + the barrier (the same 96 KB at N = 512).
 template <int N>
 __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
