@@ -48,8 +48,6 @@ void drop_graphs(fpm_ctx* ctx) {
 // carved views of the caller's workspace
 struct Workspace {
   float* rho;
-  float* rho_f;      // density mesh of the fused interleaved path: outside the interleaved force mesh, so that it can
-                     // be cleared for the next paint while the current force evaluation is still running
   float2* dk;
   float2* fk[3];
   float* F[3];
@@ -68,7 +66,6 @@ Workspace carve(const fpm_ctx* ctx) {
   //  a skew between them was measured to make no difference: DESIGN.md section 15)
   w.dk = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew;
   for (int d = 0; d < 3; ++d) { w.fk[d] = reinterpret_cast<float2*>(p); p += b * cplx_bytes(n) + kSkew; }
-  w.rho_f = reinterpret_cast<float*>(p);
   return w;
 }
 
@@ -137,23 +134,12 @@ int force_meshes(fpm_ctx* ctx, const Workspace& w, const float* pos, int64_t n, 
   cudaStream_t s = ctx->stream;
   Profiler* pr = &ctx->prof;
   const int batch = batch_of(ctx->cfg);
-  if (interleaved && ctx->cfg.force_path == FPM_FORCE_FUSED) {
-    // the density goes to its own mesh, which the x round trip clears again once the z r2c pass has read it:
-    // only the first force evaluation after fpm_set_workspace (or after a failed call) pays for a memset
-    const bool clean = ctx->rho_clean;
-    ctx->rho_clean = false;
-    { ProfScope sc(pr, K_PAINT);
-      FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho_f, !clean, order_of(ctx, n), s, batch)); }
-    FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho_f, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F, w.rho,
-                                  (float)(1.5 * ctx->cfg.omega_m), s, pr, batch, &ctx->maps, w.rho_f));
-    ctx->rho_clean = true;
-    return FPM_OK;
-  }
   { ProfScope sc(pr, K_PAINT);
     FPM_CUDA(ctx, paint(pos, nullptr, particle_mass(ctx), n, ng, w.rho, true, order_of(ctx, n), s, batch)); }
   if (ctx->cfg.force_path == FPM_FORCE_FUSED) {
     FPM_CUDA(ctx, fft_force_fused(ctx->fft_g, ctx->kt_g, w.rho, w.dk, w.fk[0], w.fk[1], w.fk[2], w.F,
-                                  nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr, batch, &ctx->maps));
+                                  interleaved ? w.rho : nullptr, (float)(1.5 * ctx->cfg.omega_m), s, pr, batch,
+                                  &ctx->maps));
     return FPM_OK;
   }
   FPM_CUDA(ctx, fft_r2c(ctx->fft_g, w.rho, w.dk, s, pr));
@@ -253,7 +239,7 @@ const char* fpm_version(void) { return "fpm-b200 0.1 (sm_100a)"; }
 
 size_t fpm_workspace_bytes(const fpm_config* cfg) {
   if (!config_ok(cfg)) return 0;
-  return (size_t)batch_of(*cfg) * (5 * real_bytes(cfg->ng) + 4 * cplx_bytes(cfg->ng)) + 4 * kSkew;
+  return (size_t)batch_of(*cfg) * (4 * real_bytes(cfg->ng) + 4 * cplx_bytes(cfg->ng)) + 4 * kSkew;
 }
 
 int fpm_create(const fpm_config* cfg, void* cuda_stream, fpm_ctx** out) {
@@ -304,7 +290,6 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
   FPM_REQUIRE(ctx, (reinterpret_cast<uintptr_t>(ws) & 255) == 0, "workspace must be 256-byte aligned");
   if (bytes < fpm_workspace_bytes(&ctx->cfg)) return fail(ctx, FPM_ENOMEM, "workspace too small");
   drop_graphs(ctx);
-  ctx->rho_clean = false;
   ctx->ws = ws;
   ctx->ws_bytes = bytes;
   const Workspace w = carve(ctx);
@@ -550,7 +535,6 @@ int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& k
     if (g.pos == pos && g.mom == mom && g.traj == traj && g.kf == kf && g.dr == dr) {
       FPM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
       ctx->prof.launches += g.launches;
-      ctx->rho_clean = true;             // (every captured run clears the density mesh itself and leaves it cleared)
       return FPM_OK;
     }
   if (!ctx->capture_stream &&
@@ -566,7 +550,6 @@ int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& k
   }
   ctx->stream = ctx->capture_stream;
   ctx->prof.stream = ctx->capture_stream;
-  ctx->rho_clean = false;                // a captured run starts with its own memset: replays do not depend on history
   const int rc = run_steps(ctx, pos, mom, kf, dr, traj);
   ctx->stream = user;
   ctx->prof.stream = user;
@@ -579,7 +562,6 @@ int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& k
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
     ctx->sticky = false;                 // a failed capture enqueued nothing; the eager path reports real errors
-    ctx->rho_clean = false;
     return FPM_ENOTIMPL;
   }
   cudaGraphDestroy(graph);
@@ -588,9 +570,7 @@ int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& k
     ctx->graphs.erase(ctx->graphs.begin());
   }
   ctx->graphs.push_back(fpm_ctx::RunGraph{pos, mom, traj, kf, dr, exec, nodes});
-  ctx->rho_clean = false;                // nothing has run yet; true again once the launch below is enqueued
   FPM_CUDA(ctx, cudaGraphLaunch(exec, ctx->stream));
-  ctx->rho_clean = true;
   ctx->prof.launches += nodes;
   return FPM_OK;
 }

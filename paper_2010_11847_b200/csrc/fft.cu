@@ -147,16 +147,9 @@ template <int N>
 cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, const float2* in, float2* out_a,
                                 float2* out_bx, float scale, bool poisson, cudaStream_t s, int batch = 1,
                                 const CUtensorMap* m_in = nullptr, const CUtensorMap* m_a = nullptr,
-                                const CUtensorMap* m_bx = nullptr, float* zero_mesh = nullptr) {
+                                const CUtensorMap* m_bx = nullptr) {
   constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N), TX = xf_tile<N>();
   const dim3 grid((nzh + TX - 1) / TX, N, batch);
-  ZeroJob zj;
-  if (zero_mesh) {      // batch meshes of N^3 floats, 16-byte aligned (N is a multiple of 4)
-    zj.ptr = reinterpret_cast<float4*>(zero_mesh);
-    zj.total = (unsigned long long)batch * N * N * N / 4;
-    const unsigned long long blocks = (unsigned long long)grid.x * grid.y * grid.z;
-    zj.per_block = (unsigned)((zj.total + blocks - 1) / blocks);
-  }
   const unsigned threads = TX * Plan<N, xf_variant<N>()>::P;
   cudaError_t e;
   // (at N = 1024 the three-buffer tile is 192 KB, one block per SM, and the ld.global version with its two
@@ -167,17 +160,17 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
       auto kern = fft_x_force_tma_kernel<N, true>;
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
-      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_a, t.stage_x, kt.lap, kt.grad, scale, zj);
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_a, t.stage_x, kt.lap, kt.grad, scale);
     } else if (tune("XPAIR", 1)) {
       auto kern = fft_x_force_pair_tma_kernel<N>;
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
-      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale, zj);
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
     } else {
       auto kern = fft_x_force_tma_kernel<N, false>;
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
-      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale, zj);
+      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
     }
     return cudaGetLastError();
   }
@@ -185,7 +178,7 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
     e = set_smem(kern, xf_smem_bytes<N>());
     if (e != cudaSuccess) return e;
     kern<<<grid, threads, xf_smem_bytes<N>(), s>>>(in, out_a, poisson ? nullptr : out_bx, nzh, PZ, t.stage_x, kt.lap,
-                                                   kt.grad, scale, zj);
+                                                   kt.grad, scale);
     return cudaGetLastError();
   };
   if (tune("XSWZ", 0) && TX == 8)
@@ -209,7 +202,7 @@ cudaError_t launch_z_r2c_padded(const FftTables& t, const float* real, float2* c
 template <int N>
 cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                              float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                             cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps, float* zero_mesh) {
+                             cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps) {
   constexpr int nzh = N / 2 + 1, PZ = padded_pitch(N);
   const bool tma = maps && maps->ok;
   // a batch of meshes back to back: its z rows and its x slabs are just more rows / slabs; only the x
@@ -246,7 +239,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   {
     ProfScope sc(prof, K_FFT_X_FORCE);
     e = launch_x_round_trip<N>(t, kt, dk, wa, wb, scale, false, s, batch, tma ? &maps->x[0] : nullptr,
-                               tma ? &maps->x[1] : nullptr, tma ? &maps->x[2] : nullptr, zero_mesh);
+                               tma ? &maps->x[1] : nullptr, tma ? &maps->x[2] : nullptr);
     if (e != cudaSuccess) return e;
   }
   {
@@ -445,9 +438,9 @@ cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float*
 
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps, float* zero_mesh) {
+                            cudaStream_t s, Profiler* prof, int batch, const TileMaps* maps) {
   if (kt.n != t.n) return cudaErrorInvalidValue;
-  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof, batch, maps, zero_mesh)
+  FPM_FFT_DISPATCH(force_fused_impl, t, kt, rho, dk, wa, wb, wc, F, F4, scale, s, prof, batch, maps)
 }
 
 }  // namespace fpm

@@ -135,38 +135,6 @@ template <int N> __host__ __device__ constexpr size_t xf_smem_bytes() {
   return sizeof(float2) * 2 * (size_t)N * xf_tile<N>();
 }
 
-// A slice of a real mesh zeroed by every block of the x round trip while it waits for its tile: the density mesh
-// of the NEXT paint (the z r2c pass of this force evaluation has consumed it).  The round trip uses 42 % of the
-// DRAM bandwidth, so the 4 n_g bytes of zeros ride along and the step needs no separate memset pass.
-struct ZeroJob {
-  float4* ptr = nullptr;            // nullptr: nothing to do
-  unsigned per_block = 0;           // float4 words per block
-  unsigned long long total = 0;     // float4 words in all
-};
-__device__ __forceinline__ void zero_slice(const ZeroJob& z) {
-  if (z.ptr == nullptr) return;
-  const unsigned long long blk = ((unsigned long long)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-  const unsigned long long i0 = blk * z.per_block;
-  const unsigned long long i1 = i0 + z.per_block < z.total ? i0 + z.per_block : z.total;
-  for (unsigned long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) z.ptr[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-}
-// The same slice written by bulk copies of a zeroed shared-memory block (one thread, async proxy: no LSU
-// wavefronts, which is what the round trip is short of; the plain stores above cost it exactly the memset's time).
-// zsrc: kZeroBlock bytes of zeros in shared memory, made visible to the async proxy by the caller; the copies join
-// the calling thread's current bulk group.
-constexpr unsigned kZeroBlock = 4096;
-__device__ __forceinline__ void zero_slice_bulk(const ZeroJob& z, const void* zsrc) {
-  if (z.ptr == nullptr) return;
-  const unsigned long long blk = ((unsigned long long)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-  const unsigned long long i0 = blk * z.per_block;
-  const unsigned long long i1 = i0 + z.per_block < z.total ? i0 + z.per_block : z.total;
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(zsrc);
-  for (unsigned long long i = i0; i < i1; i += kZeroBlock / 16) {
-    const unsigned bytes = (unsigned)((i1 - i) * 16 < kZeroBlock ? (i1 - i) * 16 : kZeroBlock);
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(z.ptr + i), "r"(sa), "r"(bytes) : "memory");
-  }
-}
-
 // POISSON: only  out_a = inverse_x[ (scale / K^2) forward_x[in] ]  (real multiplier, no gradient variant;
 // out_a may alias in) -- the x round trip of the backward pass's single potential solve.
 // grid = (ceil(nzh / T), N, batch): block (bx, y, b) owns the T columns kz = bx T .. of row y of mesh b;
@@ -176,13 +144,12 @@ __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N 
 fft_x_force_kernel(const float2* in, float2* out_a,
                    float2* __restrict__ out_bx, int nzh, int pitch,
                    const float2* __restrict__ tw, const float* __restrict__ lap,
-                   const float* __restrict__ grad, float scale, ZeroJob zj) {
+                   const float* __restrict__ grad, float scale) {
   extern __shared__ float2 smem[];
   using PL = Plan<N, xf_variant<N>()>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P;
   const int c = threadIdx.x % T, p = threadIdx.x / T;
   const int y = blockIdx.y, kz = blockIdx.x * T + c;
-  zero_slice(zj);
   const bool ok = kz < nzh;
   // blockIdx.z: mesh of a batch (meshes back to back)
   const int64_t line_stride = (int64_t)N * pitch, col = (int64_t)blockIdx.z * N * line_stride + (int64_t)y * pitch + kz;
@@ -485,7 +452,7 @@ fft_y_inv3_tma_kernel(const __grid_constant__ CUtensorMap m_bx, const __grid_con
 // stage buffer and Bx from the park buffer while the next transform runs, so no store is waited for before
 // the end.  Shared memory = [exchange | park | stage] (3 N T complex) + the barrier.
 template <int N> __host__ __device__ constexpr size_t xf_tma_smem_bytes() {
-  return sizeof(float2) * 3 * (size_t)N * xf_tile<N>() + 16 + 4096;     // + barrier + kZeroBlock
+  return sizeof(float2) * 3 * (size_t)N * xf_tile<N>() + 16;
 }
 
 // VAR: plan variant.  (The 32-points-per-thread, one-exchange plan Plan<512, 0> halves the shared-memory
@@ -494,7 +461,7 @@ template <int N, bool POISSON = false, int VAR = xf_variant<N>()>
 __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, VAR>::P, N == 512 ? 2 : 1)
 fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
                        const __grid_constant__ CUtensorMap m_bx, const float2* __restrict__ tw,
-                       const float* __restrict__ lap, const float* __restrict__ grad, float scale, ZeroJob zj) {
+                       const float* __restrict__ lap, const float* __restrict__ grad, float scale) {
   extern __shared__ __align__(128) float2 smem[];
   using PL = Plan<N, VAR>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
@@ -511,7 +478,6 @@ fft_x_force_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_co
 #pragma unroll
     for (int b = 0; b < NBOX; ++b) tma_load_3d(stage + b * BOXR * T, &m_in, col0, y, x0 + b * BOXR, bar);
   }
-  zero_slice(zj);                                       // while the tile is in flight
   mbar_wait(bar, 0);
   float2 v[E];
 #pragma unroll
@@ -577,27 +543,21 @@ template <int N>
 __global__ void __launch_bounds__(xf_tile<N>() * Plan<N, xf_variant<N>()>::P, N == 512 ? 2 : 1)
 fft_x_force_pair_tma_kernel(const __grid_constant__ CUtensorMap m_in, const __grid_constant__ CUtensorMap m_a,
                             const __grid_constant__ CUtensorMap m_bx, const float2* __restrict__ tw,
-                            const float* __restrict__ lap, const float* __restrict__ grad, float scale, ZeroJob zj) {
+                            const float* __restrict__ lap, const float* __restrict__ grad, float scale) {
   extern __shared__ __align__(128) float2 smem[];
   using PL = Plan<N, xf_variant<N>()>;
   constexpr int T = xf_tile<N>(), E = PL::E, P = PL::P, BOXR = tma_box_rows<N>(), NBOX = N / BOXR;
   float2* xch = smem;                                   // 2 N T complex: forward exchange, pair exchange, B_x stage
   float2* stage = smem + 2 * N * T;                     // N T complex: input tile, then A stage
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + 3 * N * T);
-  float4* zblock = reinterpret_cast<float4*>(smem + 3 * N * T + 2);      // kZeroBlock bytes of zeros (ZeroJob)
   const int c = threadIdx.x % T, p = threadIdx.x / T;
   const int y = blockIdx.y, col0 = blockIdx.x * T, kz = col0 + c, x0 = blockIdx.z * N;
   if (threadIdx.x == 0) mbar_init(bar, 1);
-  if (zj.ptr != nullptr) {
-    for (int i = threadIdx.x; i < (int)(kZeroBlock / 16); i += blockDim.x) zblock[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    fence_proxy_async();
-  }
   __syncthreads();
   if (threadIdx.x == 0) {
     mbar_expect_tx(bar, (unsigned)(sizeof(float2) * N * T));
 #pragma unroll
     for (int b = 0; b < NBOX; ++b) tma_load_3d(stage + b * BOXR * T, &m_in, col0, y, x0 + b * BOXR, bar);
-    zero_slice_bulk(zj, zblock);                        // joins the bulk group of the A / B_x stores below
   }
   mbar_wait(bar, 0);
   cpair w[E];

@@ -108,13 +108,10 @@ cudaError_t fft_c2r(const FftTables& t, float2* cplx, float* real, cudaStream_t 
 // paint'ed density -> the three force meshes F[0..2] with the transfer function fused into the
 // transform passes (fft.cu); scale = 1.5 omega_m (or 1).  F4 != nullptr: the three components are
 // written interleaved per cell as float4 (x, y, z, unused) into F4[4 ng^3] instead of F[0..2].
-// batch > 1 (F4 only): every buffer holds `batch` meshes back to back and each pass covers them all.
-// zero_mesh != nullptr: `batch` real meshes that the x round trip fills with zeros on the side (the density mesh
-// of the next paint; it may be `rho`, which is dead after the z r2c pass)
+// batch > 1 (F4 only): every buffer holds `batch` meshes back to back and each pass covers them all
 cudaError_t fft_force_fused(const FftTables& t, const KernelTables& kt, const float* rho, float2* dk,
                             float2* wa, float2* wb, float2* wc, float* const* F, float* F4, float scale,
-                            cudaStream_t s, Profiler* prof = nullptr, int batch = 1, const TileMaps* maps = nullptr,
-                            float* zero_mesh = nullptr);
+                            cudaStream_t s, Profiler* prof = nullptr, int batch = 1, const TileMaps* maps = nullptr);
 
 // out = c2r[(scale / K^2) r2c[src]] with the multiplier fused into the x round trip (backward pass)
 cudaError_t fft_poisson(const FftTables& t, const KernelTables& kt, const float* src, float2* work, float* out,
@@ -218,8 +215,6 @@ struct fpm_ctx {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   fpm::TileMaps maps;               // tensor maps of the workspace's half-complex meshes (fpm_set_workspace)
-  bool rho_clean = false;           // the fused path's density mesh (Workspace::rho_f) holds zeros: the x round trip
-                                    // of the last force evaluation cleared it, the next paint needs no memset
   int coarse_n = 0;                 // plans of the coarse mesh of the pyramid scheme (fpm_force_pyramid), made on demand
   fpm::FftTables fft_c;
   fpm::KernelTables kt_c;

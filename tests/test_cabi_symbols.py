@@ -42,7 +42,7 @@ def test_argument_validation_needs_no_gpu():
     lib.fpm_workspace_bytes.restype = ctypes.c_size_t
     good = Cfg(512, 512, 0.3075, 1000.0, 0, 0, 0, 0)
     nk = 512 * 512 * 272          # half-complex scratch rows are padded to 16 elements (128 bytes)
-    assert lib.fpm_workspace_bytes(ctypes.byref(good)) == 5 * 512 ** 3 * 4 + 4 * nk * 8
+    assert lib.fpm_workspace_bytes(ctypes.byref(good)) == 4 * 512 ** 3 * 4 + 4 * nk * 8
     for bad in (Cfg(500, 500, 0.3, 0, 0, 0, 0, 0), Cfg(64, 128, 0.3, 0, 0, 0, 0, 0),
                 Cfg(2048, 2048, 0.3, 0, 0, 0, 0, 0), Cfg(64, 64, -1.0, 0, 0, 0, 0, 0),
                 Cfg(64, 64, 0.3, 0, 7, 0, 0, 0), Cfg(64, 64, 0.3, 0, 0, 0, 0, 9), Cfg(64, 64, 0.3, 0, 0, 0, 5, 0),
@@ -52,7 +52,7 @@ def test_argument_validation_needs_no_gpu():
         h = ctypes.c_void_p()
         assert lib.fpm_create(ctypes.byref(bad), None, ctypes.byref(h)) == -1
     batched = Cfg(128, 128, 0.3075, 200.0, 0, 0, 1, 0, 16)
-    assert lib.fpm_workspace_bytes(ctypes.byref(batched)) == 16 * (5 * 128 ** 3 * 4 + 4 * 128 * 128 * 80 * 8)
+    assert lib.fpm_workspace_bytes(ctypes.byref(batched)) == 16 * (4 * 128 ** 3 * 4 + 4 * 128 * 128 * 80 * 8)
     assert lib.fpm_destroy(None) == -1
     assert lib.fpm_paint(None, None, None, ctypes.c_int64(0), None) == -1
     # calls added for the backward pass and N1 validate the same way
