@@ -302,6 +302,28 @@ int fpm_expand(fpm_ctx* ctx, const float* in, int levels, float* out);
  * (The factor 2^levels converts the coarse mesh's force per coarse cell spacing into fine-cell units.) */
 int fpm_force_pyramid(fpm_ctx* ctx, const float* pos, int64_t n, int levels, float* force);
 
+/* REDUCE for callers that cannot allocate device memory (no context, no workspace, no cudaMalloc anywhere on
+ * its path).  Meant for code hosted where device memory already belongs to someone else -- a plug-in inside a
+ * process whose framework pool or MIG/MPS budget holds all of it, so a fresh cudaMalloc fails or makes the pool
+ * give memory back -- and for loops that cannot afford the device-wide synchronisation an allocation implies.
+ * Same result as fpm_reduce: `levels` stride-2 convolutions, in [ng^3] -> out [(ng >> levels)^3], both DEVICE
+ * arrays of the CURRENT device owned by the caller (in != out); cuda_stream: a cudaStream_t of that device
+ * (NULL = legacy default stream); work is enqueued, not synchronised.
+ *   - The intermediates of the axis passes live in an array built into the library image,
+ *     FPM_REDUCE_STATIC_MAX_NG^3 floats = 8 MiB, which every GPU that loads libfpm's kernels holds until the
+ *     process exits.  ng > FPM_REDUCE_STATIC_MAX_NG returns FPM_EINVAL (use fpm_reduce with a workspace).
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress); make that
+ *     first call outside any stream capture.  Later calls only launch kernels.
+ *   - All calls on a device share the one array.  It is never cleared and need not be (each pass writes what
+ *     the next reads), but two calls whose kernels overlap on the GPU -- different streams, no dependency --
+ *     race on it: keep calls on one stream or order them with events.
+ * err: HOST buffer of err_len bytes receiving a message on failure ("" on success), or NULL.  Returns FPM_OK,
+ * FPM_EINVAL (pointers, ng not a power of two in [8, FPM_REDUCE_STATIC_MAX_NG], levels with ng >> levels < 8)
+ * or FPM_ECUDA. */
+#define FPM_REDUCE_STATIC_MAX_NG 128
+int fpm_reduce_static(const float* in, int ng, int levels, float* out, void* cuda_stream, char* err,
+                      size_t err_len);
+
 /* ---- measurement hooks -------------------------------------------------------------------- */
 /* Per-kernel CUDA-event timing on the context's stream (off by default).  fpm_profile_read
  * synchronises the recorded events; kernel_id runs over 0 .. until FPM_EINVAL is returned.

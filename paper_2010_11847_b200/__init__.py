@@ -84,6 +84,7 @@ def _load():
         "fpm_paint_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
         "fpm_reduce": (i32, [vp, vp, i32, vp]),
         "fpm_expand": (i32, [vp, vp, i32, vp]),
+        "fpm_reduce_static": (i32, [vp, i32, i32, vp, vp, ctypes.c_char_p, ctypes.c_size_t]),
         "fpm_force_pyramid": (i32, [vp, vp, i64, i32, vp]),
         "fpm_readout_adjoint": (i32, [vp, vp, vp, i64, vp, vp, vp]),
     }
@@ -102,6 +103,31 @@ def version():
 
 def library_path():
     return _LIB_PATH
+
+
+REDUCE_STATIC_MAX_NG = 128
+
+
+def reduce_static(mesh, levels, out):
+    """fpm_reduce_static: REDUCE `mesh` [ng^3] by `levels` levels into the caller's `out` [(ng >> levels)^3]
+    without a context, a workspace or any device allocation -- for code that runs where device memory is
+    already owned by something else (a framework pool, a fixed MIG/MPS budget) or that cannot take the
+    device-wide synchronisation of cudaMalloc.  The intermediates use an 8 MiB array built into libfpm.so
+    (meshes up to REDUCE_STATIC_MAX_NG^3; larger ones raise).  Enqueued on torch's current stream.  Calls share
+    that array: do not let two of them overlap on the GPU.  The first call on a device does a one-time address
+    lookup and should come before any stream capture.  Nothing is allocated here either: `out` is required."""
+    shape = tuple(getattr(mesh, "shape", ()))
+    if len(shape) != 3 or not (shape[0] == shape[1] == shape[2]):
+        raise FpmError(f"mesh: expected an [ng][ng][ng] tensor, got shape {shape}")
+    ng, levels = int(shape[0]), int(levels)
+    nc = ng >> levels if 0 <= levels < 8 else 0
+    err = ctypes.create_string_buffer(256)
+    rc = _lib.fpm_reduce_static(_dev(mesh, what="mesh"), ng, levels,
+                                _dev(out, numel=nc ** 3 if nc else None, what="out"),
+                                ctypes.c_void_p(torch.cuda.current_stream(mesh.device).cuda_stream), err, len(err))
+    if rc != OK:
+        raise FpmError(f"fpm_reduce_static -> {rc}: {err.value.decode()}")
+    return out
 
 
 def _dev(t, dtype=torch.float32, numel=None, what="tensor"):

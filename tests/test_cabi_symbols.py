@@ -66,3 +66,19 @@ def test_argument_validation_needs_no_gpu():
     assert lib.fpm_lpt_init_vjp(None, None, ctypes.c_double(0.1), 2, None, None, None) == -1
     assert lib.fpm_adam_step(None, None, None, None, None, ctypes.c_int64(0), ctypes.c_double(0.1),
                              ctypes.c_double(0.9), ctypes.c_double(0.999), ctypes.c_double(1e-8), 1) == -1
+
+
+def test_reduce_static_validates_without_a_gpu():
+    """fpm_reduce_static checks its arguments before it touches CUDA, and says why it refuses."""
+    from paper_2010_11847_b200 import build as fpm_build
+    lib = ctypes.CDLL(fpm_build.build())
+    vp = ctypes.c_void_p
+    lib.fpm_reduce_static.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp, vp, ctypes.c_char_p, ctypes.c_size_t]
+    err = ctypes.create_string_buffer(200)
+    a, b = vp(256), vp(512)                   # never dereferenced: every case below fails validation first
+    assert lib.fpm_reduce_static(None, 64, 1, b, None, err, len(err)) == -1 and b"distinct" in err.value
+    assert lib.fpm_reduce_static(a, 256, 1, b, None, err, len(err)) == -1
+    assert b"exceeds the built-in scratch (meshes up to 128^3)" in err.value
+    assert lib.fpm_reduce_static(a, 96, 1, b, None, err, len(err)) == -1 and b"power of two" in err.value
+    assert lib.fpm_reduce_static(a, 32, 3, b, None, err, len(err)) == -1 and b"levels" in err.value
+    assert lib.fpm_reduce_static(a, 32, 3, b, None, None, 0) == -1      # the message buffer is optional
