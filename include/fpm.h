@@ -126,10 +126,23 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes);
 /* Changes cfg.paint_mode after creation.  FPM_EINVAL on an unknown mode. */
 int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode);
 
+/* Which tile movers the fused FFT passes (FPM_FORCE_FUSED, fpm_force_vjp's potential solve) use.  The
+ * library holds exactly two chains and nothing but this call selects between them (no environment variable):
+ * FPM_MOVERS_AUTO [default] moves tiles with TMA tensor maps (cp.async.bulk.tensor) when the driver provides
+ * cuTensorMapEncodeTiled, FPM_MOVERS_GLOBAL forces the ld.global / st.global chain that otherwise runs only
+ * when it does not (same arithmetic, results equal to round-off).  fpm_tile_movers reports what the context
+ * runs now: FPM_MOVERS_TENSOR_MAPS or FPM_MOVERS_GLOBAL (the latter also before a workspace is set). */
+enum { FPM_MOVERS_AUTO = 0, FPM_MOVERS_GLOBAL = 1, FPM_MOVERS_TENSOR_MAPS = 2 };
+int fpm_set_tile_movers(fpm_ctx* ctx, int tile_movers);
+int fpm_tile_movers(const fpm_ctx* ctx);
+
 /* How fpm_nbody enqueues its n_steps + 1 PM steps.  FPM_GRAPH_AUTO [default]: when one PM step is small enough
- * to be bound by launch latency (batch * ng^3 <= 2^24 cells), the whole run is captured once into a CUDA graph
- * (cached per argument set on the context) and replayed with one launch; larger runs enqueue kernel by kernel.
- * Results are identical either way. */
+ * to be bound by launch latency (batch * ng^3 <= 2^24 cells), a run whose argument set (pos, mom, traj, schedule)
+ * repeats the previous call's is captured into a CUDA graph (cached on the context, 8 entries) and replayed
+ * with one launch from then on; a first or one-off argument set, and larger runs, enqueue kernel by kernel.
+ * FPM_GRAPH_ALWAYS captures on the first call.  When the context's stream is itself being captured by the caller
+ * (e.g. torch.cuda.graph), fpm_nbody never builds a graph of its own: it enqueues plain launches, which the
+ * caller's capture records.  Results are identical either way. */
 enum { FPM_GRAPH_OFF = 0, FPM_GRAPH_AUTO = 1, FPM_GRAPH_ALWAYS = 2 };
 int fpm_set_graph_mode(fpm_ctx* ctx, int graph_mode);
 

@@ -19,6 +19,7 @@ FACTORS_FASTPM, FACTORS_QUINN = 0, 1
 FORCE_UNFUSED, FORCE_FUSED = 0, 1
 PAINT_AUTO, PAINT_DIRECT, PAINT_BRICK_FLOAT, PAINT_BRICK_FIXED = 0, 1, 2, 3
 GRAPH_OFF, GRAPH_AUTO, GRAPH_ALWAYS = 0, 1, 2
+MOVERS_AUTO, MOVERS_GLOBAL, MOVERS_TENSOR_MAPS = 0, 1, 2
 VJP_GRAD_MOM_ZERO = 1
 OK, EINVAL, ENOMEM, ECUDA, ENOTIMPL = 0, -1, -2, -3, -4
 
@@ -51,6 +52,8 @@ def _load():
         "fpm_set_workspace": (i32, [vp, vp, ctypes.c_size_t]),
         "fpm_set_paint_mode": (i32, [vp, i32]),
         "fpm_set_graph_mode": (i32, [vp, i32]),
+        "fpm_set_tile_movers": (i32, [vp, i32]),
+        "fpm_tile_movers": (i32, [vp]),
         "fpm_growth": (i32, [vp, dbl, ctypes.POINTER(dbl)]),
         "fpm_drift_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
         "fpm_kick_factor": (i32, [vp, dbl, dbl, dbl, ctypes.POINTER(dbl)]),
@@ -209,6 +212,12 @@ class FPM:
 
     def set_graph_mode(self, mode):
         self._check(_lib.fpm_set_graph_mode(self._h, int(mode)))
+
+    def set_tile_movers(self, mode):
+        self._check(_lib.fpm_set_tile_movers(self._h, int(mode)))
+
+    def tile_movers(self):
+        return int(_lib.fpm_tile_movers(self._h))
 
     # ---- cosmology ----------------------------------------------------------------------
     def growth(self, a):
@@ -464,6 +473,7 @@ class FPM:
         return (loss[0], loss[1]), grad
 
     def adam_step(self, x, grad, m, v, lr, t, beta1=0.9, beta2=0.999, eps=1e-8):
-        self._check(_lib.fpm_adam_step(self._h, _dev(x), _dev(grad), _dev(m), _dev(v), x.numel(), lr, beta1,
-                                       beta2, eps, int(t)))
+        n = x.numel()
+        self._check(_lib.fpm_adam_step(self._h, _dev(x), _dev(grad, numel=n, what="grad"), _dev(m, numel=n, what="m"),
+                                       _dev(v, numel=n, what="v"), n, lr, beta1, beta2, eps, int(t)))
         return x

@@ -34,8 +34,8 @@ bool config_ok(const fpm_config* c) {
   return true;
 }
 
-// bytes between consecutive half-complex buffers (A/B knob; measured to make no difference, so 0)
-const size_t kSkew = (size_t)256 * (size_t)tune("SKEW256", 0);
+// bytes between consecutive half-complex buffers (a skew was measured to make no difference: DESIGN.md 15)
+constexpr size_t kSkew = 0;
 
 inline int batch_of(const fpm_config& c) { return c.batch > 1 ? c.batch : 1; }
 
@@ -295,7 +295,27 @@ int fpm_set_workspace(fpm_ctx* ctx, void* ws, size_t bytes) {
   const Workspace w = carve(ctx);
   float2* const bufs[4] = {w.dk, w.fk[0], w.fk[1], w.fk[2]};
   FPM_CUDA(ctx, fft_make_tile_maps(ctx->cfg.ng, batch_of(ctx->cfg), bufs, &ctx->maps));
+  if (ctx->tile_movers == FPM_MOVERS_GLOBAL) ctx->maps.ok = false;
   return FPM_OK;
+}
+
+int fpm_set_tile_movers(fpm_ctx* ctx, int tile_movers) {
+  FPM_ENTER(ctx);
+  FPM_REQUIRE(ctx, tile_movers == FPM_MOVERS_AUTO || tile_movers == FPM_MOVERS_GLOBAL, "unknown tile mover mode");
+  drop_graphs(ctx);
+  ctx->tile_movers = tile_movers;
+  if (ctx->ws) {
+    const Workspace w = carve(ctx);
+    float2* const bufs[4] = {w.dk, w.fk[0], w.fk[1], w.fk[2]};
+    FPM_CUDA(ctx, fft_make_tile_maps(ctx->cfg.ng, batch_of(ctx->cfg), bufs, &ctx->maps));
+  }
+  if (tile_movers == FPM_MOVERS_GLOBAL) ctx->maps.ok = false;
+  return FPM_OK;
+}
+
+int fpm_tile_movers(const fpm_ctx* ctx) {
+  if (!ctx) return FPM_EINVAL;
+  return ctx->ws && ctx->maps.ok ? FPM_MOVERS_TENSOR_MAPS : FPM_MOVERS_GLOBAL;
 }
 
 int fpm_set_paint_mode(fpm_ctx* ctx, int paint_mode) {
@@ -414,6 +434,7 @@ const float* fpm_workspace_density(const fpm_ctx* ctx) {
 int fpm_kick(fpm_ctx* ctx, float* mom, const float* force, int64_t n, double ai, double ac,
              double af) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_kick");
   FPM_REQUIRE(ctx, n >= 0 && ((mom && force) || n == 0), "fpm_kick: bad arguments");
   FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_kick: scale factors must be positive");
   const double k = kick_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
@@ -425,6 +446,7 @@ int fpm_kick(fpm_ctx* ctx, float* mom, const float* force, int64_t n, double ai,
 int fpm_drift(fpm_ctx* ctx, float* pos, const float* mom, int64_t n, double ai, double ac,
               double af) {
   FPM_ENTER(ctx);
+  FPM_NO_BATCH(ctx, "fpm_drift");
   FPM_REQUIRE(ctx, n >= 0 && ((pos && mom) || n == 0), "fpm_drift: bad arguments");
   FPM_REQUIRE(ctx, ai > 0.0 && ac > 0.0 && af > 0.0, "fpm_drift: scale factors must be positive");
   const double d = drift_factor(ctx->cfg.omega_m, ai, ac, af, ctx->cfg.factor_mode);
@@ -527,16 +549,27 @@ int run_steps(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& k
 // The same run as ONE CUDA graph launch (fpm.h FPM_GRAPH_*): a small configuration spends its step in launch
 // latency (C1: 8 launches of 6-24 us for 0.1 ms of work), so the run is captured once -- on an internal stream:
 // the caller's may be the legacy default stream, which cannot be captured -- and replayed on ctx->stream.
-// Graphs are cached per (pos, mom, traj, factors).  Returns FPM_ENOTIMPL when capture is not possible (the
-// caller then enqueues kernel by kernel); nothing has been enqueued in that case.
+// Graphs are cached per (pos, mom, traj, factors).  Capture + instantiation cost more than the launches one
+// replay saves, so under FPM_GRAPH_AUTO an argument set is captured only the second time in a row it is seen
+// (`always` = FPM_GRAPH_ALWAYS captures at once).  Returns FPM_ENOTIMPL when no graph is used or capture is not
+// possible (the caller then enqueues kernel by kernel); nothing has been enqueued in that case.
 int run_graph(fpm_ctx* ctx, float* pos, float* mom, const std::vector<double>& kf, const std::vector<double>& dr,
-              float* traj) {
+              float* traj, bool always) {
   for (auto& g : ctx->graphs)
     if (g.pos == pos && g.mom == mom && g.traj == traj && g.kf == kf && g.dr == dr) {
       FPM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
       ctx->prof.launches += g.launches;
       return FPM_OK;
     }
+  if (!always) {
+    auto& sn = ctx->seen;
+    const bool again = sn.valid && sn.pos == pos && sn.mom == mom && sn.traj == traj && sn.kf == kf && sn.dr == dr;
+    if (!again) {
+      sn.pos = pos; sn.mom = mom; sn.traj = traj; sn.kf = kf; sn.dr = dr; sn.valid = true;
+      return FPM_ENOTIMPL;
+    }
+    sn.valid = false;
+  }
   if (!ctx->capture_stream &&
       cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
     cudaGetLastError();
@@ -591,8 +624,17 @@ int fpm_nbody(fpm_ctx* ctx, float* pos, float* mom, const double* a_stages, int 
   const int64_t cells = (int64_t)batch_of(ctx->cfg) * ctx->cfg.ng * ctx->cfg.ng * ctx->cfg.ng;
   const bool want_graph = ctx->graph_mode == FPM_GRAPH_ALWAYS ||
                           (ctx->graph_mode == FPM_GRAPH_AUTO && cells <= (int64_t(1) << 24));
-  if (want_graph && !ctx->prof.enabled) {          // (per-kernel event timing needs the kernel-by-kernel path)
-    const int rc = run_graph(ctx, pos, mom, kf, dr, traj);
+  // Inside the CALLER's own stream capture (e.g. torch.cuda.graph) the run must stay plain launches on
+  // ctx->stream, which the caller's graph then records: creating a stream, capturing or instantiating here could
+  // be refused or invalidate that capture.  (On the legacy default stream the query itself fails while another
+  // stream captures in global mode -- without harming that capture; treated the same way.)
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(ctx->stream, &cap) != cudaSuccess) {
+    cudaGetLastError();
+    cap = cudaStreamCaptureStatusActive;
+  }
+  if (want_graph && !ctx->prof.enabled && cap == cudaStreamCaptureStatusNone) {   // (event timing needs kernel by kernel)
+    const int rc = run_graph(ctx, pos, mom, kf, dr, traj, ctx->graph_mode == FPM_GRAPH_ALWAYS);
     if (rc != FPM_ENOTIMPL) return rc;
   }
   return run_steps(ctx, pos, mom, kf, dr, traj);

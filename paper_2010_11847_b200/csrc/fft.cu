@@ -103,7 +103,7 @@ cudaError_t launch_z_c2r(const FftTables& t, const float2* cplx, float* real, co
   const float scale = (float)(1.0 / ((double)N * N * N));
   const unsigned grid = (unsigned)((nrows + G - 1) / G);
   // bulk row loads need whole blocks of an even number of rows (16-byte aligned runs)
-  const bool tma = G % 2 == 0 && nrows % G == 0 && (reinterpret_cast<uintptr_t>(cplx) & 15) == 0 && tune("ZTMA", 1);
+  const bool tma = G % 2 == 0 && nrows % G == 0 && (reinterpret_cast<uintptr_t>(cplx) & 15) == 0;
   cudaError_t e;
   if (tma) {
     auto kern = fft_z_c2r_kernel<N, true>;
@@ -154,20 +154,15 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
   cudaError_t e;
   // (at N = 1024 the three-buffer tile is 192 KB, one block per SM, and the ld.global version with its two
   //  64 KB buffers is faster: 6.1 vs 6.7 ms at C5)
-  if (m_in && m_a && (poisson || m_bx) && tune("TMA", N <= 512 ? 1 : 0)) {     // TMA tile movers
+  if (m_in && m_a && (poisson || m_bx) && N <= 512) {     // TMA tile movers
     const size_t smem = xf_tma_smem_bytes<N>();
     if (poisson) {
       auto kern = fft_x_force_tma_kernel<N, true>;
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
       kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_a, t.stage_x, kt.lap, kt.grad, scale);
-    } else if (tune("XPAIR", 1)) {
-      auto kern = fft_x_force_pair_tma_kernel<N>;
-      e = set_smem(kern, smem);
-      if (e != cudaSuccess) return e;
-      kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
     } else {
-      auto kern = fft_x_force_tma_kernel<N, false>;
+      auto kern = fft_x_force_pair_tma_kernel<N>;
       e = set_smem(kern, smem);
       if (e != cudaSuccess) return e;
       kern<<<grid, threads, smem, s>>>(*m_in, *m_a, *m_bx, t.stage_x, kt.lap, kt.grad, scale);
@@ -181,8 +176,6 @@ cudaError_t launch_x_round_trip(const FftTables& t, const KernelTables& kt, cons
                                                    kt.grad, scale);
     return cudaGetLastError();
   };
-  if (tune("XSWZ", 0) && TX == 8)
-    return poisson ? go(fft_x_force_kernel<N, true, true>) : go(fft_x_force_kernel<N, false, true>);
   return poisson ? go(fft_x_force_kernel<N, true, false>) : go(fft_x_force_kernel<N, false, false>);
 }
 
@@ -218,7 +211,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
   }
   {
     ProfScope sc(prof, K_FFT_Y);
-    if (tma && tune("TMA", 1) && tune("YFWD_TMA", 1)) {
+    if (tma) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = sizeof(float2) * N * TY + 16;
       dim3 grid((nzh + TY - 1) / TY, slabs);
@@ -229,8 +222,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
                                                   yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
         e = cudaGetLastError();
       };
-      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 6 : 1)>);
-      else go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 2 : 1)>);
+      go(fft_y_inv3_tma_kernel<N, false, (N == 512 ? 6 : 1)>);
     } else {
       e = launch_cols<N, false>(dk, dk, slabs, (int64_t)N * PZ, nzh, PZ, t.stage_n, s);
     }
@@ -246,7 +238,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
     ProfScope sc(prof, K_FFT_Y_INV3);
     using YPL = Plan<N, yi_variant<N>()>;
     // Fx: wb in place; Fy: g_y A -> dk (free now); Fz: A -> wc
-    if (tma && tune("TMA", 1)) {
+    if (tma) {
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = sizeof(float2) * N * TY + 16;
       dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
@@ -256,10 +248,9 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
         kern<<<grid, yi_threads<N>(), ysmem, s>>>(maps->y[2], maps->y[1], maps->y[0], maps->y[3],
                                                   yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad, 0);
       };
-      if (N == 512 && tune("YOCC", 3) == 3) go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 6 : 1)>);
-      else go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 2 : 1)>);
+      go(fft_y_inv3_tma_kernel<N, true, (N == 512 ? 6 : 1)>);
       if (e != cudaSuccess) return e;
-    } else if (tune("YPAIR", 1)) {
+    } else {                    // no tensor maps: the ld.global column-pair pass
       constexpr int TY = yi_tile<N>();
       const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
       auto kern = fft_y_inv3_pair_kernel<N>;
@@ -268,15 +259,6 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
       dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
       kern<<<grid, yi_threads<N>(), ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * PZ, nzh, PZ,
                                                 yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
-    } else {
-      constexpr int TY = yi1_tile<N>();
-      const size_t ysmem = YPL::NST > 1 ? sizeof(float2) * N * TY : 0;
-      auto kern = fft_y_inv3_kernel<N>;
-      e = set_smem(kern, ysmem);
-      if (e != cudaSuccess) return e;
-      dim3 grid(3 * ((nzh + TY - 1) / TY), slabs);
-      kern<<<grid, TY * YPL::P, ysmem, s>>>(wb, wa, wb, dk, wc, (int64_t)N * PZ, nzh, PZ,
-                                            yi_variant<N>() ? t.stage_x : t.stage_n, kt.grad);
     }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -293,7 +275,7 @@ cudaError_t force_fused_impl(const FftTables& t, const KernelTables& kt, const f
           (float)(1.0 / ((double)N * N * N)), kt.grad);
       return cudaGetLastError();
     };
-    return tune("ZTMA", 1) ? go(fft_z_c2r3_kernel<N, true>) : go(fft_z_c2r3_kernel<N, false>);
+    return go(fft_z_c2r3_kernel<N, true>);
   }
   e = launch_z_c2r<N>(t, wb, F[0], nullptr, s, prof, PZ);
   if (e != cudaSuccess) return e;

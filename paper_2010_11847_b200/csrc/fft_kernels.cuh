@@ -240,42 +240,6 @@ fft_y_inv3_pair_kernel(const float2* in_bx, const float2* __restrict__ in_a, flo
   }
 }
 
-// the same pass with one column per thread (8-byte accesses; 8-column tiles at N = 512)
-template <int N> __host__ __device__ constexpr int yi1_tile() { return N == 512 ? 8 : col_tile<N>(); }
-
-template <int N>
-__global__ void __launch_bounds__(yi1_tile<N>() * Plan<N, yi_variant<N>()>::P)
-fft_y_inv3_kernel(const float2* in_bx, const float2* __restrict__ in_a, float2* out_x,
-                  float2* __restrict__ out_y, float2* __restrict__ out_z, int64_t batch_stride,
-                  int ncols, int64_t line_stride, const float2* __restrict__ tw,
-                  const float* __restrict__ grad) {
-  extern __shared__ float2 smem[];
-  using PL = Plan<N, yi_variant<N>()>;
-  constexpr int T = yi1_tile<N>(), E = PL::E, P = PL::P;
-  const int c = threadIdx.x % T, p = threadIdx.x / T;
-  const int variant = blockIdx.x % 3;
-  const int64_t col = (int64_t)(blockIdx.x / 3) * T + c;
-  const bool ok = col < ncols;
-  const int64_t off = (int64_t)blockIdx.y * batch_stride + col;
-  const float2* in = variant == 0 ? in_bx : in_a;
-  float2* out = variant == 0 ? out_x : (variant == 1 ? out_y : out_z);
-  float2 v[E];
-#pragma unroll
-  for (int e = 0; e < E; ++e) {
-    const int i = p + P * e;
-    float2 x = make_float2(0.f, 0.f);
-    if (ok) x = in[off + (int64_t)i * line_stride];
-    if (variant == 1) { const float g = __ldg(grad + i); x.x *= g; x.y *= g; }
-    v[e] = cswap(x);
-  }
-  ColSmem<T, true> sm{smem, c};
-  fft_line_plan<PL>(v, p, sm, tw);
-  if (ok) {
-#pragma unroll
-    for (int e = 0; e < E; ++e) out[off + (int64_t)(p + P * e) * line_stride] = cswap(v[e]);
-  }
-}
-
 // real rows of N floats -> rows of N/2+1 complex.  twn[k] = exp(-2 pi i k / N), k < N/2.
 template <int N>
 __global__ void __launch_bounds__(z_rows<N>() * Plan<N / 2>::P)

@@ -57,10 +57,6 @@ using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn encode_tiled_fn();
 
-// Tuning switches for A/B measurements (environment FPM_TUNE_<NAME>, read once); the defaults are the
-// measured winners and the product never depends on a switch being set.
-int tune(const char* name, int dflt);     // profiler.cpp
-
 // ---- FFT (fft.cu) ---------------------------------------------------------------------------
 struct FftTables {
   int n = 0;
@@ -215,6 +211,7 @@ struct fpm_ctx {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   fpm::TileMaps maps;               // tensor maps of the workspace's half-complex meshes (fpm_set_workspace)
+  int tile_movers = FPM_MOVERS_AUTO; // FPM_MOVERS_GLOBAL: maps.ok is kept false (fpm_set_tile_movers)
   int coarse_n = 0;                 // plans of the coarse mesh of the pyramid scheme (fpm_force_pyramid), made on demand
   fpm::FftTables fft_c;
   fpm::KernelTables kt_c;
@@ -232,4 +229,7 @@ struct fpm_ctx {
     long long launches;
   };
   std::vector<RunGraph> graphs;
+  // the argument set of the last fpm_nbody call that missed the cache under FPM_GRAPH_AUTO: a run is captured
+  // only when the same set comes back (a caller with fresh buffers every call never pays for a capture)
+  struct { float *pos = nullptr, *mom = nullptr, *traj = nullptr; std::vector<double> kf, dr; bool valid = false; } seen;
 };

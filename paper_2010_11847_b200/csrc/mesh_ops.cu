@@ -807,10 +807,7 @@ cudaError_t paint(const float* pos, const float* mass, float mass_const, int64_t
     return mass ? go(paint_brick_kernel<false, true, 2>) : go(paint_brick_kernel<false, false, 2>);
   }
   if (mode == FPM_PAINT_BRICK_FIXED) {
-    static const bool xmerge = !(std::getenv("FPM_TUNE_XMERGE") && std::getenv("FPM_TUNE_XMERGE")[0] == '0');
-    if (xmerge && !mass && tune("PAINT_OCC", 3) == 3) return go(paint_brick_kernel<true, false, 1, true, 3>);
-    if (xmerge) return mass ? go(paint_brick_kernel<true, true, 1, true>) : go(paint_brick_kernel<true, false, 1, true>);
-    return mass ? go(paint_brick_kernel<true, true>) : go(paint_brick_kernel<true, false>);
+    return mass ? go(paint_brick_kernel<true, true, 1, true>) : go(paint_brick_kernel<true, false, 1, true, 3>);
   }
   return mass ? go(paint_brick_kernel<false, true>) : go(paint_brick_kernel<false, false>);
 }

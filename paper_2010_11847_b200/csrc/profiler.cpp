@@ -24,19 +24,6 @@ EncodeTiledFn encode_tiled_fn() {
   return fn;
 }
 
-int tune(const char* name, int dflt) {
-  static std::mutex mu;
-  static std::map<std::string, int> cache;
-  std::lock_guard<std::mutex> lock(mu);
-  auto it = cache.find(name);
-  if (it != cache.end()) return it->second;
-  const std::string key = std::string("FPM_TUNE_") + name;
-  const char* v = std::getenv(key.c_str());
-  const int val = v ? std::atoi(v) : dflt;
-  cache[name] = val;
-  return val;
-}
-
 // (kernel, device) pairs whose MaxDynamicSharedMemorySize attribute is already raised to >= bytes
 cudaError_t ensure_dynamic_smem_impl(const void* kernel, size_t bytes) {
   static std::mutex mu;

@@ -89,6 +89,39 @@ def test_force_evaluation_matches_oracle(fpm, oracle, ng, nps, mode, force_path)
     assert np.max(np.abs(got.astype(np.float64).sum(axis=1))) < 1e-4 * np.sqrt(np.mean(ref ** 2)) * n
 
 
+@pytest.mark.parametrize("ng,nps,mode", [(64, 64, 0), (64, 32, 1), (128, 128, 0), (128, 64, 2)])
+def test_fused_force_through_the_global_tile_movers_matches_oracle(fpm, oracle, ng, nps, mode):
+    """The chain a driver without cuTensorMapEncodeTiled gets (fpm_set_tile_movers(FPM_MOVERS_GLOBAL): forward y
+    by launch_cols, fft_x_force_kernel, fft_y_inv3_pair_kernel), against the oracle like the default chain --
+    both the planar force meshes (fpm_force) and the interleaved mesh of the step kernels (fpm_pm_step) -- and
+    the potential solve of fpm_force_vjp through the same movers."""
+    import torch
+    n = nps ** 3
+    pos = fi.random_particles(n, ng, seed=ng + mode, clustered=True)
+    ctx = fpm.FPM(ng, nps, kernel_mode=mode, force_path=fpm.FORCE_FUSED)
+    assert ctx.tile_movers() == fpm.MOVERS_TENSOR_MAPS          # what a B200 driver provides
+    ctx.set_tile_movers(fpm.MOVERS_GLOBAL)
+    assert ctx.tile_movers() == fpm.MOVERS_GLOBAL
+    mass = float((ng // nps) ** 3)
+    ref = oracle.force(pos.astype(np.float64), ng, mode=mode, scale=1.5 * OM, mass=mass)
+    d_pos = dev(pos)
+    planar = host(ctx.force(d_pos))
+    step = torch.zeros_like(d_pos)
+    ctx.pm_step(d_pos.clone(), step, 1.0, 0.0)                  # mom = 0 + f(pos) * 1
+    for got in (planar, host(step)):
+        assert rel_l2(got, ref) < 1e-5
+        assert np.max(np.abs(got - ref)) < 1e-5 * np.max(np.abs(ref))
+    v = np.random.default_rng(5).standard_normal((3, n)).astype(np.float32)
+    got = host(ctx.force_vjp(d_pos, dev(v), coef=0.37))
+    ref = 0.37 * oracle.force_vjp(pos.astype(np.float64), ng, v.astype(np.float64), mode=mode, scale=1.5 * OM, mass=mass)
+    assert rel_l2(got, ref) < 1e-4
+    ctx.set_tile_movers(fpm.MOVERS_AUTO)
+    assert ctx.tile_movers() == fpm.MOVERS_TENSOR_MAPS
+    assert rel_l2(host(ctx.force(d_pos)), planar) < 1e-6
+    with pytest.raises(fpm.FpmError):
+        ctx.set_tile_movers(7)
+
+
 def test_zero_force_on_lattice(fpm):
     for ng, nps in ((32, 32), (32, 16)):
         b = ng // nps

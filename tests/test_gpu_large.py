@@ -157,9 +157,11 @@ def test_fused_passes_with_the_512_plan_variants_match_the_oracle(fpm, oracle):
         d_pos = dev(pos)
         f_step = host(force_through_the_step_kernels(ctx, d_pos)).astype(np.float64)   # interleaved mesh
         f_planar = host(ctx.force(d_pos)).astype(np.float64)                            # planar c2r path
+        ctx.set_tile_movers(fpm.MOVERS_GLOBAL)                                          # the chain without tensor maps
+        f_global = host(force_through_the_step_kernels(ctx, d_pos)).astype(np.float64)
         ctx.close()
         ref = oracle.force(pos.astype(np.float64), ng, mode=mode, scale=1.5 * OM, mass=float((ng // nps) ** 3))
-        for got in (f_step, f_planar):
+        for got in (f_step, f_planar, f_global):
             assert rel_l2(got, ref) < 1e-5
             assert np.max(np.abs(got - ref)) < 1e-5 * np.max(np.abs(ref))
 

@@ -64,6 +64,19 @@ def test_adam_step_matches_oracle(fpm, oracle):
     assert rel_l2(host(dx), rx) < 1e-6 and rel_l2(host(dm), rm) < 1e-6 and rel_l2(host(dv), rv) < 1e-6
 
 
+def test_adam_step_refuses_short_state_tensors(fpm):
+    """grad, m and v are indexed up to x.numel() behind the C-ABI: a short one must be refused by the binding."""
+    import torch
+    ctx = fpm.FPM(16)
+    x = torch.zeros(4096, device="cuda")
+    ok = torch.zeros(4096, device="cuda")
+    short = torch.zeros(4095, device="cuda")
+    for args in ((short, ok, ok), (ok, short, ok), (ok, ok, short)):
+        with pytest.raises(fpm.FpmError, match="expected 4096 elements"):
+            ctx.adam_step(x, *args, 0.1, 1)
+    ctx.adam_step(x, ok, ok.clone(), ok.clone(), 0.1, 1)
+
+
 def test_reconstruction_loop_descends_like_the_oracle(fpm, oracle):
     """12 Adam iterations from s = 0 (Listing 7.1 train loop): GPU and oracle losses track each other."""
     import torch
