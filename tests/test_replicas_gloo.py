@@ -78,7 +78,8 @@ def test_bench_style_self_launch_of_two_replicas(tmp_path):
         "assert not rep.needs_spawn(int(sys.argv[1]))\n"
         "rank, local, world = rep.init('gloo')\n"
         "ms = rep.max_over_ranks(1.0 + rank)\n"
-        "print('RANK', rank, world, rep.replica_seed(1, rank), ms, flush=True)\n"
+        "sys.stdout.write(f'RANK {rank} {world} {rep.replica_seed(1, rank)} {ms}\\n')\n"     # one write: the ranks share a pipe
+        "sys.stdout.flush()\n"
         "rep.finalize()\n")
     cmd = rep.launch_command(2, str(script), ["2"])
     assert "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
