@@ -334,3 +334,27 @@ def test_C3_gradient_lands_on_the_stored_oracle_gradient(fpm):
     assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 2e-2
     assert pct[0] < 2e-3 * rms                             # the typical lattice point agrees far better than the tail
     assert float(torch.linalg.vector_norm(gd.double())) == pytest.approx(norms["grad_l2"], rel=1e-3)
+
+
+def test_force_vjp_at_512_matches_the_oracle_on_the_same_positions(fpm, oracle):
+    """R12 at the benchmark's mesh size: one fpm_force_vjp on the 512^3 mesh (128^3 clustered
+    particles, so B = 4 bricks are not used and the oracle's reverse pass stays at a few FFTs of 512^3) against
+    oracle.force_vjp on the SAME fp32 positions and cotangent.  Pins the N = 512 instantiations of the backward
+    chain -- the direct dW/dx gather, the three cotangent paints, stencil_divergence_kernel and the fused
+    potential solve fft_poisson -- at the operator tolerance of test_gpu_backward.py (1e-4) instead of the
+    2e-2 / 5 % the end-to-end gradient checks at C3 / C4 can give along their own fp32 trajectories."""
+    nps, ng = 128, 512
+    n = nps ** 3
+    pos = fi.random_particles(n, ng, seed=31, clustered=True)
+    v = np.random.default_rng(32).standard_normal((3, n)).astype(np.float32)
+    mass = float((ng // nps) ** 3)
+    ctx = fpm.FPM(ng, nps, omega_m=OM, force_path=fpm.FORCE_FUSED)
+    got = host(ctx.force_vjp(dev(pos), dev(v), coef=0.37)).astype(np.float64)
+    ctx.set_tile_movers(fpm.MOVERS_GLOBAL)
+    got_global = host(ctx.force_vjp(dev(pos), dev(v), coef=0.37)).astype(np.float64)
+    ctx.close()
+    ref = 0.37 * oracle.force_vjp(pos.astype(np.float64), ng, v.astype(np.float64), scale=1.5 * OM, mass=mass)
+    print(f"force VJP at 512^3: rel-L2 {rel_l2(got, ref):.2e} (tensor maps), {rel_l2(got_global, ref):.2e} (ld.global); "
+          f"max-abs {np.max(np.abs(got - ref)):.2e} of {np.max(np.abs(ref)):.2e}")
+    assert rel_l2(got, ref) < 1e-4 and rel_l2(got_global, ref) < 1e-4
+    assert np.max(np.abs(got - ref)) < 1e-4 * np.max(np.abs(ref))
